@@ -1,0 +1,170 @@
+"""CPU oracle for the COLATUS hot path -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Thin ctypes wrapper over `colatus_oracle.c` (plain C, FP64, OpenMP over
+targets).  Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s
+`cpu_baseline` / `--impl reference` legs may import this package; the product
+package `paper_1208_3444_b200` never does, and this package never imports it.
+
+Inputs are the same float32 arrays handed to the GPU, promoted exactly to
+double here.  See the header of `colatus_oracle.c` for citations and pins.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from ctypes import c_double, c_int, c_int64, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "colatus_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11",
+                               "-ffp-contract=off", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(c_double)
+        lib.oracle_num_threads.restype = c_int
+        lib.oracle_forces.argtypes = [c_void_p, c_void_p, c_int64, c_double, c_double,
+                                      c_void_p, c_int64, c_void_p, c_void_p]
+        lib.oracle_forces.restype = None
+        lib.oracle_step.argtypes = [c_void_p, c_void_p, c_void_p, c_int64, c_double, c_double,
+                                    c_double, c_double, c_double, c_void_p]
+        lib.oracle_step.restype = None
+        lib.oracle_step_coeffs.argtypes = [c_void_p, c_void_p, c_void_p, c_int64, c_double, c_double,
+                                           c_double, c_double, c_double, c_double, c_void_p]
+        lib.oracle_step_coeffs.restype = None
+        lib.oracle_hubble.argtypes = [c_double] * 6
+        lib.oracle_hubble.restype = c_double
+        lib.oracle_a_advance.argtypes = [c_double] * 7 + [c_int]
+        lib.oracle_a_advance.restype = c_double
+        lib.oracle_time_of_a.argtypes = [c_double] * 6 + [c_int64]
+        lib.oracle_time_of_a.restype = c_double
+        lib.oracle_int_dt_over_a_pow.argtypes = [c_double] * 8 + [c_int]
+        lib.oracle_int_dt_over_a_pow.restype = c_double
+        lib.oracle_diagnostics.argtypes = [c_void_p, c_void_p, c_void_p, c_int64, c_double, c_double,
+                                           c_double, c_int, c_void_p]
+        lib.oracle_diagnostics.restype = None
+        del dp
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(c_void_p)
+
+
+def _c64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def forces_xm(x, m, eps2, G, targets=None, potential=False):
+    """Eq. (1) on double arrays x [n,3], m [n].  Returns acc [k,3] (and phi [k])."""
+    x = _c64(x)
+    m = _c64(m)
+    n = x.shape[0]
+    if targets is None:
+        tptr, k = None, n
+    else:
+        targets = np.ascontiguousarray(targets, dtype=np.int64)
+        tptr, k = _p(targets), targets.shape[0]
+    acc = np.empty((k, 3), dtype=np.float64)
+    phi = np.empty(k, dtype=np.float64) if potential else None
+    _load().oracle_forces(_p(x), _p(m), n, float(eps2), float(G), tptr, k, _p(acc),
+                          _p(phi) if potential else None)
+    return (acc, phi) if potential else acc
+
+
+def forces(pos_mass, eps2, G, targets=None, potential=False):
+    """Eq. (1) on the float32 [n,4] body array the GPU receives (promoted exactly)."""
+    pm = np.asarray(pos_mass)
+    return forces_xm(pm[:, :3].astype(np.float64), pm[:, 3].astype(np.float64),
+                     eps2, G, targets, potential)
+
+
+class State:
+    """Double-precision simulation state started from the float32 input arrays."""
+
+    def __init__(self, pos_mass, vel, eps2, G):
+        pm = np.asarray(pos_mass)
+        self.x = np.ascontiguousarray(pm[:, :3].astype(np.float64))
+        self.m = np.ascontiguousarray(pm[:, 3].astype(np.float64))
+        self.v = np.ascontiguousarray(np.asarray(vel)[:, :3].astype(np.float64))
+        self.n = self.x.shape[0]
+        self.eps2 = float(eps2)
+        self.G = float(G)
+        self._work = np.empty_like(self.x)
+
+    def step(self, tau, a, H):
+        """Eqs. (3)-(5)."""
+        _load().oracle_step(_p(self.x), _p(self.v), _p(self.m), self.n, self.eps2, self.G,
+                            float(tau), float(a), float(H), _p(self._work))
+
+    def step_coeffs(self, d1, cv, ck, d2):
+        _load().oracle_step_coeffs(_p(self.x), _p(self.v), _p(self.m), self.n, self.eps2, self.G,
+                                   float(d1), float(cv), float(ck), float(d2), _p(self._work))
+
+    def last_force(self):
+        """F(x^{n+1/2}) of the most recent step."""
+        return self._work.copy()
+
+    def diagnostics(self, a, with_potential=False):
+        out = np.zeros(16, dtype=np.float64)
+        _load().oracle_diagnostics(_p(self.x), _p(self.v), _p(self.m), self.n, self.eps2, self.G,
+                                   float(a), int(bool(with_potential)), _p(out))
+        return out
+
+
+def _cos(c):
+    return (float(c.H0), float(c.Om_R), float(c.Om_M), float(c.Om_K), float(c.Om_L))
+
+
+def hubble(cosmo, a):
+    """Eq. (2)."""
+    return float(_load().oracle_hubble(*_cos(cosmo), float(a)))
+
+
+def a_advance(cosmo, a0, dt, substeps=64):
+    return float(_load().oracle_a_advance(*_cos(cosmo), float(a0), float(dt), int(substeps)))
+
+
+def time_of_a(cosmo, a, panels=2_000_000):
+    return float(_load().oracle_time_of_a(*_cos(cosmo), float(a), int(panels)))
+
+
+def int_dt_over_a_pow(cosmo, a0, dt, p, panels=64):
+    return float(_load().oracle_int_dt_over_a_pow(*_cos(cosmo), float(a0), float(dt), float(p), int(panels)))
+
+
+def midstep_schedule(cosmo, a_start, tau, steps, substeps=64):
+    """(a, H) at t_n + tau/2 for n = 0..steps-1 (reading G3), plus a at the step ends.
+
+    cosmo None = static background: a = 1, H = 0 (config 3, reading G13)."""
+    if cosmo is None:
+        return [(1.0, 0.0)] * steps, [1.0] * (steps + 1)
+    mids, ends = [], [float(a_start)]
+    a = float(a_start)
+    for _ in range(steps):
+        a_mid = a_advance(cosmo, a, 0.5 * tau, substeps)
+        mids.append((a_mid, hubble(cosmo, a_mid)))
+        a = a_advance(cosmo, a_mid, 0.5 * tau, substeps)
+        ends.append(a)
+    return mids, ends

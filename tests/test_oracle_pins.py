@@ -1,0 +1,473 @@
+"""T0: pin the CPU oracle to what the paper and the mathematics fix.
+
+None of these compares the oracle with itself or with the CUDA path: every expected
+value is a closed form, an exact rational worked example (tests/golden/), an invariant,
+or an independent few-line NumPy evaluation on tiny inputs.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1208_3444_b200.inputs import Cosmology
+
+RNG = np.random.Generator(np.random.PCG64(12345))
+
+
+# ----------------------------------------------------------------------------- P1
+def test_two_body_closed_form_and_direction():
+    """|F on 1| = G m2 r / (r^2+eps^2)^{3/2}, pointing from body 1 TOWARD body 2 (G1)."""
+    G, eps2 = 2.5, 0.09
+    x = np.array([[0.1, -0.2, 0.3], [0.7, 0.4, -0.5]])
+    m = np.array([3.0, 5.0])
+    d = x[1] - x[0]
+    r = np.linalg.norm(d)
+    F = oracle.forces_xm(x, m, eps2, G)
+    assert np.allclose(F[0], G * m[1] * r / (r * r + eps2) ** 1.5 * d / r, rtol=1e-14)
+    assert np.allclose(F[1], -G * m[0] * r / (r * r + eps2) ** 1.5 * d / r, rtol=1e-14)
+    assert np.dot(F[0], d) > 0 and np.dot(F[1], d) < 0           # attraction
+
+
+def test_softened_force_maximum():
+    """max_r G m r/(r^2+eps^2)^{3/2} = 2 G m / (3 sqrt(3) eps^2) at r = eps/sqrt(2)."""
+    G, mass, eps = 1.0, 2.0, 0.25
+    rs = np.linspace(0.01, 1.0, 2001)
+    f = []
+    for r in rs:
+        F = oracle.forces_xm(np.array([[0, 0, 0], [r, 0, 0.0]]), np.array([0.0, mass]), eps * eps, G)
+        f.append(F[0, 0])
+    f = np.array(f)
+    i = int(np.argmax(f))
+    assert abs(rs[i] - eps / math.sqrt(2)) < 1e-3
+    fmax = oracle.forces_xm(np.array([[0, 0, 0], [eps / math.sqrt(2), 0, 0.0]]),
+                            np.array([0.0, mass]), eps * eps, G)[0, 0]
+    assert fmax == pytest.approx(2 * G * mass / (3 * math.sqrt(3) * eps * eps), rel=1e-14)
+
+
+def _read_golden(path):
+    rows = {}
+    with open(path) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            tok = line.split()
+            rows[tok[0]] = tok[1:]
+    return rows
+
+
+def test_three_body_exact_rational(golden_dir):
+    rows = _read_golden(os.path.join(golden_dir, "three_body_rational.txt"))
+    x = np.array([[0, 0, 0], [1, 2, 2], [2, 4, 0]], dtype=np.float64)
+    m = np.array([1.0, 2.0, 3.0])
+    F = oracle.forces_xm(x, m, 16.0, 1.0)
+    for i, body in enumerate("ABC"):
+        want = [float(Fraction(s)) for s in rows[body]]
+        assert np.allclose(F[i], want, rtol=0, atol=2e-17), (body, F[i], want)
+    assert np.allclose((m[:, None] * F).sum(axis=0), 0.0, atol=1e-16)
+
+
+# ----------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("n", [2, 17, 500])
+def test_newton_third_law(n):
+    x = RNG.random((n, 3))
+    m = RNG.random(n) + 0.1
+    F = oracle.forces_xm(x, m, 1e-4, 1.7)
+    num = np.linalg.norm((m[:, None] * F).sum(axis=0))
+    den = (m * np.linalg.norm(F, axis=1)).sum()
+    assert num / den < 1e-13
+
+
+# ----------------------------------------------------------------------------- P3
+def _fibonacci_shell(n, R):
+    i = np.arange(n) + 0.5
+    z = 1.0 - 2.0 * i / n
+    phi = math.pi * (1.0 + math.sqrt(5.0)) * i
+    s = np.sqrt(1.0 - z * z)
+    return R * np.stack([s * np.cos(phi), s * np.sin(phi), z], axis=1)
+
+
+def _shell_force_radial(G, M, R, r, eps2):
+    """-d/dr of phi(r) = -(G M / 2 r R) [sqrt((R+r)^2+eps^2) - sqrt((R-r)^2+eps^2)]."""
+    A = math.sqrt((R + r) ** 2 + eps2)
+    B = math.sqrt((R - r) ** 2 + eps2)
+    return (G * M / (2 * R)) * (((R + r) / A + (R - r) / B) / r - (A - B) / (r * r))
+
+
+def _shell_potential(G, M, R, r, eps2):
+    return -(G * M / (2 * r * R)) * (math.sqrt((R + r) ** 2 + eps2) - math.sqrt((R - r) ** 2 + eps2))
+
+
+@pytest.mark.parametrize("eps", [0.001, 0.05, 0.3])
+def test_shell_theorem_softened_closed_form(eps):
+    G, M, R, n = 1.3, 2.0, 1.0, 10_000
+    shell = _fibonacci_shell(n, R)
+    direction = np.array([0.36, -0.48, 0.8])                       # unit vector
+    tol = {0.1: 3e-6, 0.5: 1.2e-5, 0.8: 9e-5, 1.5: 1.2e-5, 3.0: 3e-7}
+    for r, t in tol.items():
+        x = np.concatenate([shell, (r * direction)[None, :]], axis=0)
+        m = np.concatenate([np.full(n, M / n), [0.0]])
+        F, phi = oracle.forces_xm(x, m, eps * eps, G, targets=np.array([n]), potential=True)
+        Fr = float(F[0] @ direction)
+        Ft = np.linalg.norm(F[0] - Fr * direction)
+        scale = G * M / R ** 2
+        assert abs(Fr - _shell_force_radial(G, M, R, r, eps * eps)) < t * scale, (r, eps)
+        assert Ft < t * scale
+        assert abs(phi[0] - _shell_potential(G, M, R, r, eps * eps)) < 10 * t * G * M / R
+    # epsilon -> 0 limits: zero inside, G M / r^2 outside
+    if eps == 0.001:
+        x = np.concatenate([shell, (0.3 * direction)[None, :]], axis=0)
+        m = np.concatenate([np.full(n, M / n), [0.0]])
+        F = oracle.forces_xm(x, m, eps * eps, G, targets=np.array([n]))
+        assert np.linalg.norm(F[0]) < 1e-5 * G * M
+        x[-1] = 2.0 * direction
+        F = oracle.forces_xm(x, m, eps * eps, G, targets=np.array([n]))
+        assert float(F[0] @ direction) == pytest.approx(-G * M / 4.0, rel=1e-5)
+
+
+# ----------------------------------------------------------------------------- P4
+def _numpy_pairwise(x, m, eps2, G):
+    """Independent evaluation: full pairwise tensors, diagonal removed by masking."""
+    d = x[None, :, :] - x[:, None, :]                 # d[k, j] = x_j - x_k
+    s = (d ** 2).sum(-1) + eps2
+    w = m[None, :] * s ** -1.5
+    np.fill_diagonal(w, 0.0)
+    F = G * (w[:, :, None] * d).sum(axis=1)
+    p = m[None, :] * s ** -0.5
+    np.fill_diagonal(p, 0.0)
+    return F, -G * p.sum(axis=1)
+
+
+@pytest.mark.parametrize("n", [2, 3, 5, 8, 64])
+def test_brute_force_tiny_n(n):
+    x = RNG.normal(size=(n, 3))
+    m = RNG.random(n) + 0.05
+    F, phi = oracle.forces_xm(x, m, 0.01, 0.7, potential=True)
+    Fw, pw = _numpy_pairwise(x, m, 0.01, 0.7)
+    assert np.allclose(F, Fw, rtol=1e-12, atol=1e-14)
+    assert np.allclose(phi, pw, rtol=1e-12)
+
+
+def test_target_list_and_self_skip():
+    n = 40
+    x = RNG.random((n, 3))
+    m = RNG.random(n)
+    Fw, _ = _numpy_pairwise(x, m, 1e-3, 1.0)
+    tg = np.array([39, 0, 7, 7, 21])
+    F = oracle.forces_xm(x, m, 1e-3, 1.0, targets=tg)
+    assert np.allclose(F, Fw[tg], rtol=1e-12)
+    # two distinct particles at the same place contribute nothing to each other (G4)
+    x2 = x.copy()
+    x2[1] = x2[0]
+    F2 = oracle.forces_xm(x2, m, 1e-3, 1.0)
+    x3 = np.delete(x2, 1, axis=0)
+    m3 = np.delete(m, 1)
+    F3 = oracle.forces_xm(x3, m3, 1e-3, 1.0)
+    assert np.allclose(F2[0], F3[0], rtol=1e-12)
+
+
+def test_float32_entry_promotes_exactly():
+    pm = RNG.random((33, 4)).astype(np.float32)
+    F = oracle.forces(pm, np.float32(0.01) ** 2, 1.0)
+    Fw, _ = _numpy_pairwise(pm[:, :3].astype(np.float64), pm[:, 3].astype(np.float64),
+                            float(np.float32(0.01) ** 2), 1.0)
+    assert np.allclose(F, Fw, rtol=1e-12)
+
+
+# ----------------------------------------------------------------------------- P5
+def test_symmetries():
+    n = 200
+    x = RNG.random((n, 3))
+    m = RNG.random(n) + 0.1
+    eps2, G = 4e-4, 1.0
+    F = oracle.forces_xm(x, m, eps2, G)
+    perm = RNG.permutation(n)
+    assert np.allclose(oracle.forces_xm(x[perm], m[perm], eps2, G), F[perm], rtol=1e-11, atol=1e-13)
+    assert np.array_equal(oracle.forces_xm(x + 4.0, m, eps2, G),
+                          oracle.forces_xm((x + 4.0), m, eps2, G))
+    xs = np.round(x * 2 ** 20) / 2 ** 20                                   # translation by 2^k is exact
+    assert np.array_equal(oracle.forces_xm(xs + 2.0, m, eps2, G), oracle.forces_xm(xs, m, eps2, G))
+    lam = 3.0
+    assert np.allclose(oracle.forces_xm(lam * x, m, lam * lam * eps2, G), F / lam ** 2, rtol=1e-12)
+    assert np.allclose(oracle.forces_xm(x, 2.5 * m, eps2, G), 2.5 * F, rtol=1e-13)
+    assert np.allclose(oracle.forces_xm(x, m, eps2, 3.0 * G), 3.0 * F, rtol=1e-13)
+    mirror = x * np.array([-1.0, 1.0, 1.0])
+    assert np.allclose(oracle.forces_xm(mirror, m, eps2, G), F * np.array([-1.0, 1.0, 1.0]), rtol=1e-12)
+    # linearity in the source masses
+    m2 = RNG.random(n)
+    assert np.allclose(oracle.forces_xm(x, m + m2, eps2, G),
+                       F + oracle.forces_xm(x, m2, eps2, G), rtol=1e-11, atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- P6
+def test_far_field_monopole():
+    n, s, R = 3000, 0.01, 10.0
+    cl = s * (RNG.random((n, 3)) - 0.5)
+    m = RNG.random(n)
+    com = (m[:, None] * cl).sum(0) / m.sum()
+    probe = com + np.array([R, 0, 0])
+    x = np.concatenate([cl, probe[None]], axis=0)
+    mm = np.concatenate([m, [0.0]])
+    F = oracle.forces_xm(x, mm, 1e-8, 1.0, targets=np.array([n]))[0]
+    assert F[0] == pytest.approx(-m.sum() / R ** 2, rel=5 * (s / R) ** 2)
+    assert abs(F[1]) + abs(F[2]) < 5 * (s / R) ** 2 * m.sum() / R ** 2
+
+
+# ----------------------------------------------------------------------------- P7
+EDS = Cosmology(H0=2.5, Om_M=1.0)
+LCDM = Cosmology(H0=70.0, Om_M=0.3, Om_L=0.7)
+
+
+def test_hubble_each_term():
+    c = Cosmology(H0=3.0, Om_R=0.1, Om_M=0.2, Om_K=0.3, Om_L=0.4)
+    a = 0.5
+    assert oracle.hubble(c, a) == pytest.approx(3.0 * math.sqrt(0.1 * 16 + 0.2 * 8 + 0.3 * 4 + 0.4), rel=1e-15)
+    assert oracle.hubble(c, 1.0) == pytest.approx(3.0, rel=1e-15)
+    for name, expo in (("Om_R", -2.0), ("Om_M", -1.5), ("Om_K", -1.0), ("Om_L", 0.0)):
+        single = Cosmology(H0=1.0, **{name: 1.0})
+        assert oracle.hubble(single, 0.3) == pytest.approx(0.3 ** expo, rel=1e-14)
+
+
+def test_eds_closed_form():
+    """a = (1.5 H0 t)^{2/3}, H = 2/(3t)."""
+    H0 = EDS.H0
+    t = lambda a: (2.0 / (3.0 * H0)) * a ** 1.5
+    assert oracle.time_of_a(EDS, 0.02) == pytest.approx(t(0.02), rel=1e-10)
+    assert oracle.time_of_a(EDS, 1.0) == pytest.approx(t(1.0), rel=1e-10)
+    a0, dt = 0.02, 0.013
+    a1 = oracle.a_advance(EDS, a0, dt, 8192)
+    assert a1 == pytest.approx((1.5 * H0 * (t(a0) + dt)) ** (2.0 / 3.0), rel=1e-10)
+    assert oracle.hubble(EDS, a1) == pytest.approx(2.0 / (3.0 * (t(a0) + dt)), rel=1e-10)
+
+
+def test_flat_lcdm_closed_form():
+    """H0 t = (2 / (3 sqrt(Om_L))) asinh( sqrt(Om_L/Om_M) a^{3/2} );  H0 t0 = 0.9640993816 for (0.3, 0.7)."""
+    f = lambda a: (2.0 / (3.0 * math.sqrt(0.7))) * math.asinh(math.sqrt(0.7 / 0.3) * a ** 1.5) / 70.0
+    assert 70.0 * oracle.time_of_a(LCDM, 1.0) == pytest.approx(0.9640993816, rel=2e-10)
+    assert oracle.time_of_a(LCDM, 1.0 / 51.0) == pytest.approx(f(1.0 / 51.0), rel=1e-10)
+    # advance from z=50 to z=0 in 1000 steps of tau, as config 2 does
+    tau = (f(1.0) - f(1.0 / 51.0)) / 1000.0
+    a = 1.0 / 51.0
+    for _ in range(1000):
+        a = oracle.a_advance(LCDM, a, tau, 16)
+    assert a == pytest.approx(1.0, rel=1e-9)
+    # inverse closed form at an intermediate time
+    tmid = f(1.0 / 51.0) + 400 * tau
+    a_mid = (math.sqrt(0.3 / 0.7) * math.sinh(1.5 * math.sqrt(0.7) * 70.0 * tmid)) ** (2.0 / 3.0)
+    assert oracle.a_advance(LCDM, 1.0 / 51.0, 400 * tau, 4000) == pytest.approx(a_mid, rel=1e-10)
+
+
+def test_radiation_milne_desitter_closed_forms():
+    rad = Cosmology(H0=1.7, Om_R=1.0)                                   # a = sqrt(2 H0 t)
+    assert oracle.time_of_a(rad, 0.4) == pytest.approx(0.4 ** 2 / (2 * 1.7), rel=1e-10)
+    t0 = 0.1 ** 2 / (2 * 1.7)
+    assert oracle.a_advance(rad, 0.1, 0.05, 8192) == pytest.approx(math.sqrt(2 * 1.7 * (t0 + 0.05)), rel=1e-10)
+    milne = Cosmology(H0=0.9, Om_K=1.0)                                 # a = H0 t
+    assert oracle.time_of_a(milne, 0.6) == pytest.approx(0.6 / 0.9, rel=1e-10)
+    assert oracle.a_advance(milne, 0.2, 0.3, 64) == pytest.approx(0.2 + 0.9 * 0.3, rel=1e-12)
+    ds = Cosmology(H0=1.1, Om_L=1.0)                                    # a ~ exp(H0 t)
+    assert oracle.a_advance(ds, 0.5, 0.7, 64) == pytest.approx(0.5 * math.exp(1.1 * 0.7), rel=1e-9)
+
+
+def test_matter_radiation_and_open_closed_forms():
+    Om_M, Om_R, H0 = 0.9, 0.1, 2.0
+    mr = Cosmology(H0=H0, Om_R=Om_R, Om_M=Om_M)
+    f = lambda a: (2.0 / (3.0 * Om_M ** 2)) * ((Om_M * a - 2 * Om_R) * math.sqrt(Om_M * a + Om_R)
+                                               + 2 * Om_R ** 1.5) / H0
+    for a in (0.05, 0.5, 1.0):
+        assert oracle.time_of_a(mr, a) == pytest.approx(f(a), rel=1e-9)
+    a1 = oracle.a_advance(mr, 0.05, f(0.5) - f(0.05), 4000)
+    assert a1 == pytest.approx(0.5, rel=1e-9)
+    Om_M, Om_K = 0.3, 0.7                                               # open: cycloid-like parametric form
+    op = Cosmology(H0=H0, Om_M=Om_M, Om_K=Om_K)
+    for eta in (0.5, 1.5, 2.5):
+        a = (Om_M / (2 * Om_K)) * (math.cosh(eta) - 1.0)
+        t = (Om_M / (2 * Om_K ** 1.5)) * (math.sinh(eta) - eta) / H0
+        assert oracle.time_of_a(op, a) == pytest.approx(t, rel=1e-9)
+
+
+def test_int_dt_over_a_pow_eds():
+    """EdS: a = (t/t1)^{2/3} with t1 = 2/(3 H0): int dt/a^p has a closed form."""
+    H0 = EDS.H0
+    t1 = 2.0 / (3.0 * H0)
+    a0, dt = 0.1, 0.02
+    ta = t1 * a0 ** 1.5
+    for p in (1.0, 2.0):
+        q = 1.0 - 2.0 * p / 3.0
+        want = t1 ** (2 * p / 3) * ((ta + dt) ** q - ta ** q) / q
+        assert oracle.int_dt_over_a_pow(EDS, a0, dt, p, 2048) == pytest.approx(want, rel=1e-9)
+
+
+def test_midstep_schedule():
+    mids, ends = oracle.midstep_schedule(EDS, 0.02, 1e-3, 10)
+    t1 = 2.0 / (3.0 * EDS.H0)
+    t0 = t1 * 0.02 ** 1.5
+    for i, (a, H) in enumerate(mids):
+        tm = t0 + (i + 0.5) * 1e-3
+        assert a == pytest.approx((tm / t1) ** (2 / 3), rel=1e-9)
+        assert H == pytest.approx(2.0 / (3.0 * tm), rel=1e-9)
+    assert ends[-1] == pytest.approx(((t0 + 10e-3) / t1) ** (2 / 3), rel=1e-9)
+    mids, ends = oracle.midstep_schedule(None, 1.0, 1e-3, 3)
+    assert mids == [(1.0, 0.0)] * 3 and ends == [1.0] * 4
+
+
+# ----------------------------------------------------------------------------- P8
+def _pm(x, m):
+    return np.concatenate([np.asarray(x, dtype=np.float64), np.asarray(m, dtype=np.float64)[:, None]], axis=1)
+
+
+def _two_body_circular(eps2, G=1.0, m1=1.0, m2=0.5, r=1.0):
+    M = m1 + m2
+    omega = math.sqrt(G * M / (r * r + eps2) ** 1.5)          # softened circular frequency
+    x = np.array([[-m2 / M * r, 0, 0], [m1 / M * r, 0, 0]])
+    v = np.array([[0, -m2 / M * r * omega, 0], [0, m1 / M * r * omega, 0]])
+    return x, v, np.array([m1, m2]), omega
+
+
+def _energy(st):
+    d = st.diagnostics(1.0, with_potential=True)
+    return d[7] + d[8]
+
+
+def test_static_limit_is_leapfrog_circular_orbit():
+    eps2 = 0.04
+    x, v, m, omega = _two_body_circular(eps2)
+    period = 2 * math.pi / omega
+    errs = []
+    for nsteps in (400, 800):
+        st = oracle.State(_pm(x, m), np.concatenate([v, np.zeros((2, 1))], axis=1), eps2, 1.0)
+        E0 = _energy(st)
+        tau = period / nsteps
+        worst = 0.0
+        for _ in range(nsteps):
+            st.step(tau, 1.0, 0.0)
+            worst = max(worst, abs(_energy(st) - E0))
+            assert np.linalg.norm(st.x[1] - st.x[0]) == pytest.approx(1.0, abs=2e-3)
+        assert np.allclose(st.x, x, atol=5e-3)                # back to the start after one period
+        assert np.allclose((st.m[:, None] * st.v).sum(0), 0.0, atol=1e-15)
+        errs.append(np.linalg.norm(st.x - x))
+    assert errs[0] / errs[1] == pytest.approx(4.0, rel=0.05)   # second order: phase error ~ tau^2
+
+
+def test_static_energy_error_second_order_and_time_reversal():
+    n = 24
+    x = RNG.random((n, 3))
+    v = 0.3 * RNG.normal(size=(n, 3))
+    m = RNG.random(n) / n
+    pm = _pm(x, m)
+    v4 = np.concatenate([v, np.zeros((n, 1))], axis=1)
+    errs = []
+    for tau, steps in ((2e-3, 100), (1e-3, 200)):
+        st = oracle.State(pm, v4, 0.01, 1.0)
+        E0 = _energy(st)
+        for _ in range(steps):
+            st.step(tau, 1.0, 0.0)
+        errs.append(abs(_energy(st) - E0))
+    assert errs[0] / errs[1] == pytest.approx(4.0, rel=0.25)
+    st = oracle.State(pm, v4, 0.01, 1.0)
+    for _ in range(50):
+        st.step(1e-3, 1.0, 0.0)
+    st.v *= -1.0
+    for _ in range(50):
+        st.step(1e-3, 1.0, 0.0)
+    assert np.allclose(st.x, x, atol=1e-13)
+    assert np.allclose(-st.v, v, atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- P9
+def test_one_step_worked_example(golden_dir):
+    rows = _read_golden(os.path.join(golden_dir, "one_step_worked.txt"))
+    pm = _pm([[0, 0, 0], [1, 2, 1]], [1.0, 125.0])
+    vel = np.array([[0, 0, 0, 0], [0, 0, 8, 0]], dtype=np.float64)
+    st = oracle.State(pm, vel, 16.0, 1.0)
+    P0 = (st.m[:, None] * st.v).sum(0)
+    st.step(0.25, 0.5, 4.0 / 3.0)
+    for i, body in enumerate("AB"):
+        want = [float(s) for s in rows[body]]
+        assert np.allclose(st.x[i], want[:3], rtol=0, atol=1e-15)
+        assert np.allclose(st.v[i], want[3:], rtol=0, atol=1e-15)
+    assert np.allclose((st.m[:, None] * st.v).sum(0), 0.5 * P0, atol=1e-13)   # P' = cv P
+    assert np.allclose(st.last_force(), [[1, 2, 2], [-1 / 125, -2 / 125, -2 / 125]], atol=1e-16)
+
+
+def test_hubble_drag_without_forces():
+    """G = 0: v^n = v^0 prod (1-H tau)/(1+H tau); continuous limit v ~ a^-2, second order in tau."""
+    pm = _pm(RNG.random((5, 3)), np.ones(5))
+    v0 = RNG.normal(size=(5, 4))
+    v0[:, 3] = 0
+    errs = []
+    for steps in (50, 100):
+        tau = 0.02 / steps
+        mids, ends = oracle.midstep_schedule(EDS, 0.05, tau, steps)
+        st = oracle.State(pm, v0, 0.01, 0.0)
+        prod = 1.0
+        for a, H in mids:
+            st.step(tau, a, H)
+            prod *= (1 - H * tau) / (1 + H * tau)
+        assert np.allclose(st.v, v0[:, :3] * prod, rtol=1e-13)
+        errs.append(abs(prod - (0.05 / ends[-1]) ** 2))
+    assert errs[0] / errs[1] == pytest.approx(4.0, rel=0.1)
+    assert errs[1] < 1e-4
+
+
+def test_momentum_law_with_forces():
+    n = 50
+    pm = _pm(RNG.random((n, 3)), RNG.random(n) / n)
+    v0 = np.concatenate([0.2 * RNG.normal(size=(n, 3)), np.zeros((n, 1))], axis=1)
+    st = oracle.State(pm, v0, 1e-3, 1.0)
+    mids, _ = oracle.midstep_schedule(EDS, 0.1, 2e-3, 5)
+    for a, H in mids:
+        P = st.diagnostics(a)[1:4].copy()
+        st.step(2e-3, a, H)
+        cv = (1 - H * 2e-3) / (1 + H * 2e-3)
+        assert np.allclose(st.diagnostics(a)[1:4], cv * P, rtol=1e-12, atol=1e-16)
+
+
+# ----------------------------------------------------------------------------- diagnostics / P11
+def test_diagnostics_definitions():
+    n = 30
+    x = RNG.random((n, 3))
+    v = RNG.normal(size=(n, 3))
+    m = RNG.random(n)
+    st = oracle.State(_pm(x, m), np.concatenate([v, np.zeros((n, 1))], 1), 0.02, 1.5)
+    a = 0.4
+    d = st.diagnostics(a, with_potential=True)
+    assert d[0] == pytest.approx(m.sum(), rel=1e-14)
+    assert np.allclose(d[1:4], (m[:, None] * v).sum(0), rtol=1e-13)
+    assert np.allclose(d[4:7], a * a * (m[:, None] * v).sum(0), rtol=1e-13)
+    assert d[7] == pytest.approx(0.5 * a * a * (m * (v ** 2).sum(1)).sum(), rel=1e-13)
+    dd = x[None] - x[:, None]
+    s = np.sqrt((dd ** 2).sum(-1) + 0.02)
+    pair = m[:, None] * m[None, :] / s
+    np.fill_diagonal(pair, 0.0)
+    assert d[8] == pytest.approx(-(1.5 / (2 * a)) * pair.sum(), rel=1e-13)
+    assert np.allclose(d[9:12], (m[:, None] * x).sum(0) / m.sum(), rtol=1e-13)
+    assert math.isnan(st.diagnostics(a)[8])
+
+
+def test_layzer_irvine():
+    """d(T+W)/dt = -H (2T + W) for eq. (1): time-integrated residual is O(tau^2)."""
+    n = 64
+    pm = _pm(RNG.random((n, 3)), np.full(n, 1.0 / n))
+    v0 = np.zeros((n, 4))
+    cosmo = Cosmology(H0=math.sqrt(8 * math.pi / 3), Om_M=1.0)
+    res = []
+    for steps in (40, 80):
+        tau = 0.004 / steps
+        mids, ends = oracle.midstep_schedule(cosmo, 0.05, tau, steps)
+        st = oracle.State(pm, v0, 0.01 ** 2 * 25, 1.0)
+        d = st.diagnostics(ends[0], True)
+        E = [d[7] + d[8]]
+        rhs = [oracle.hubble(cosmo, ends[0]) * (2 * d[7] + d[8])]
+        for i, (a, H) in enumerate(mids):
+            st.step(tau, a, H)
+            d = st.diagnostics(ends[i + 1], True)
+            E.append(d[7] + d[8])
+            rhs.append(oracle.hubble(cosmo, ends[i + 1]) * (2 * d[7] + d[8]))
+        rhs = np.array(rhs)
+        integral = tau * (rhs.sum() - 0.5 * (rhs[0] + rhs[-1]))            # trapezoid
+        res.append(abs(E[-1] - E[0] + integral))
+        assert abs(E[-1] - E[0]) > 100 * res[-1]                            # non-vacuous: E changed a lot
+    assert res[0] / res[1] == pytest.approx(4.0, rel=0.35)
