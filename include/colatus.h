@@ -1,0 +1,196 @@
+/*
+ * colatus.h -- C ABI of libcolatus: the B200 (sm_100a) hot path of COLATUS,
+ * arXiv 1208.3444 ("PAPER.md" below = /root/reference/PAPER.md).
+ *
+ * What the library computes
+ *   - eq. (1), PAPER.md:29 : softened direct-summation acceleration
+ *         F_k = G * sum_{j != k} m_j (x_j - x_k) / (|x_j - x_k|^2 + eps^2)^{3/2}
+ *     (attractive sign, reading G1; the a^-3 of eq. (1) is applied in
+ *     the kick, reading G5).  FP32 arithmetic, blocked FP32 accumulation.
+ *   - eqs. (3)-(5), PAPER.md:38-44 : comoving drift-kick-drift leapfrog with the
+ *     Hubble-drag factor (1-H tau)/(1+H tau); kick and second half-drift fused.
+ *   - eq. (2), PAPER.md:33 : Friedmann equation, host only, double precision.
+ *   - per-step velocities of selected tracer particles.
+ *   - momentum / energy reductions (p = m a^2 v, eq. (7)).
+ *
+ * Conventions
+ *   - "body array" = float4 per particle, 16-byte aligned: positions carry
+ *     (x, y, z, m) -- mass in .w as in the paper's kernel, PAPER.md:142 --
+ *     velocities (vx, vy, vz, unused) and accelerations (ax, ay, az, w).
+ *   - `*_dev` pointers are DEVICE pointers owned by the caller; `*_host`
+ *     pointers are host pointers owned by the caller.  The library never
+ *     allocates or frees device memory: scratch comes from the caller's
+ *     workspace (colatus_workspace_bytes).  It keeps raw pointers only between
+ *     colatus_upload / colatus_trace and colatus_shutdown.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - One implicit process-wide context (one GPU per process).  Calls are not
+ *     thread-safe; serialise them.
+ *   - Every function returning int returns COLATUS_OK (0) or a negative
+ *     colatus_status; on error no output is written and colatus_last_error()
+ *     describes the failure.  No exception or abort crosses the ABI.
+ *   - There is no CPU fallback: without an sm_100 device colatus_init returns
+ *     COLATUS_UNSUPPORTED_DEVICE or COLATUS_CUDA_ERROR.
+ *   - Device data are not scanned: NaN/Inf inputs give NaN outputs, not errors.
+ *   - Results are bit-reproducible run to run for a fixed (n, device, build):
+ *     no floating-point atomics anywhere.
+ */
+#ifndef COLATUS_H
+#define COLATUS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum colatus_status {
+    COLATUS_OK = 0,
+    COLATUS_INVALID_ARG = -1,          /* null / misaligned pointer, n out of range, non-finite scalar ... */
+    COLATUS_NOT_INITIALISED = -2,
+    COLATUS_ALREADY_INITIALISED = -3,
+    COLATUS_WORKSPACE_TOO_SMALL = -4,
+    COLATUS_NOT_UPLOADED = -5,
+    COLATUS_UNSUPPORTED_DEVICE = -6,   /* device is not compute capability 10.x */
+    COLATUS_CUDA_ERROR = -7            /* text in colatus_last_error() */
+} colatus_status;
+
+/* colatus_config.flags */
+#define COLATUS_FLAG_NONE 0u
+
+typedef struct colatus_config {
+    double   G;                 /* gravitational constant of eq. (1); finite */
+    int      device;            /* CUDA device ordinal */
+    void    *workspace_dev;     /* device scratch, 256-byte aligned, caller-owned */
+    size_t   workspace_bytes;   /* >= colatus_workspace_bytes(n_max) for the largest n used */
+    unsigned flags;             /* COLATUS_FLAG_* */
+} colatus_config;
+
+/* Bytes of device workspace needed for problems up to n_max bodies: the repacked
+ * source array, source-split partial sums, reduction scratch, and staging for the
+ * host-buffer entry point.  Pure host arithmetic; 0 if n_max < 1. */
+size_t colatus_workspace_bytes(int64_t n_max);
+
+/* Selects the device, checks it is cc 10.x, records G and the workspace.  A second
+ * call without colatus_shutdown returns COLATUS_ALREADY_INITIALISED. */
+int  colatus_init(const colatus_config *cfg);
+void colatus_shutdown(void);
+
+/* ---- eq. (1): stateless force evaluation on caller-owned device arrays -------------
+ * pos_mass_dev : const float4[n]  (x, y, z, m)
+ * acc_out_dev  : float4[n]        (F_x, F_y, F_z, 0)  with G applied, a^-3 NOT applied
+ * eps2         : eps^2 (the paper's min_dist^2), finite, >= 1e-30
+ * Enqueues on cuda_stream and returns without synchronising.  n in [1, 2^31-1];
+ * pointers 16-byte aligned and distinct. */
+int colatus_forces(const void *pos_mass_dev, int64_t n, float eps2, void *acc_out_dev,
+                   void *cuda_stream);
+
+/* As colatus_forces but acc_out[k].w = phi_k = -G sum_{j != k} m_j / sqrt(r^2 + eps^2)
+ * (the potential whose gradient is eq. (1); used for the energy of eq. (7)). */
+int colatus_forces_potential(const void *pos_mass_dev, int64_t n, float eps2, void *acc_out_dev,
+                             void *cuda_stream);
+
+/* Forces on targets [target_begin, target_begin + target_count) only, all n bodies acting
+ * as sources; acc_out_dev is float4[target_count].  The multi-GPU path shards eq. (1) by
+ * targets with this call. */
+int colatus_forces_range(const void *pos_mass_dev, int64_t n, int64_t target_begin,
+                         int64_t target_count, float eps2, void *acc_out_dev, void *cuda_stream);
+
+/* Host-buffer variant: copies float4[n] host -> device, evaluates eq. (1), copies
+ * float4[n] back and synchronises.  Uses the workspace staging area and the stream given
+ * (NULL = default).  This is the end-to-end call bench.py's "e2e" times. */
+int colatus_forces_host(const float *pos_mass_host, int64_t n, float eps2, float *acc_out_host,
+                        void *cuda_stream);
+
+/* ---- eqs. (3)-(5): resident simulation state ----------------------------------------
+ * Binds caller-owned device buffers (float4[n] each); all later step work is enqueued
+ * on `cuda_stream`.  Resets the step counter to 0.  acc_dev receives F(x^{n+1/2}) of
+ * the latest step. */
+int colatus_upload(void *pos_mass_dev, void *vel_dev, void *acc_dev, int64_t n, float eps2,
+                   void *cuda_stream);
+
+/* One step of eqs. (3)-(5) with constant tau:
+ *   x += tau/2 v;  F = eq.(1)(x);  v = v (1-H tau)/(1+H tau) + F tau/(a^3 (1+H tau));  x += tau/2 v
+ * a, H are the caller's mid-step values (reading G3); the coefficients are formed in
+ * double on the host and passed to the kernels as float.  Requires finite arguments,
+ * a > 0 and 1 + H tau > 0.  Asynchronous. */
+int colatus_step(double tau, double a, double H);
+
+/* Generic drift-kick-drift:  x += d1 v;  F = eq.(1)(x);  v = cv v + ck F;  x += d2 v.
+ * Covers the symplectic operators of eq. (9), with v standing for p/m.
+ * Asynchronous. */
+int colatus_step_coeffs(double d1, double cv, double ck, double d2);
+
+/* Restrict the resident state to targets [target_begin, target_begin+target_count): only
+ * those bodies are drifted, kicked and receive forces; all n bodies stay sources.  Used by
+ * the target-sharded multi-GPU driver, which all-gathers positions between steps.
+ * Default after colatus_upload is the full range. */
+int colatus_set_target_range(int64_t target_begin, int64_t target_count);
+
+/* Drift alone (eq. (3)): x += d v on the resident state's target range.  Asynchronous. */
+int colatus_drift(double d);
+/* Force on the resident state's target range into acc_dev, then the fused kick-drift
+ * (eqs. (4)-(5)) v = cv v + ck F; x += d2 v and the tracer record.  Asynchronous. */
+int colatus_force_kick_drift(double cv, double ck, double d2);
+
+/* ---- tracers -------------------------------------------------
+ * After each step the velocities v^{n+1} of the k particles idx_dev[0..k) are written to
+ * ring_dev[(step % capacity_steps)][k] as float4 (vx, vy, vz, tag) where tag is the
+ * `trace_tag` of that step (colatus_step passes a as float; step_coeffs passes 0).
+ * k = 0 disables tracing.  idx_dev: const int32[k]; ring_dev: float4[capacity_steps][k]. */
+int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_steps);
+
+/* Copies steps [first_step, first_step+n_steps) of the ring to host_out[n_steps][k][4];
+ * fails with COLATUS_INVALID_ARG if the ring no longer (or not yet) holds them.
+ * Synchronises the stream. */
+int colatus_trace_read(float *host_out, int64_t first_step, int n_steps);
+
+/* ---- diagnostics (eq. (7)) ------------------------------
+ * out[0] = M = sum m;  out[1..3] = P = sum m v;  out[4..6] = a^2 P;
+ * out[7] = T = 1/2 sum m a^2 v^2;  out[8] = W = -(G/2a) sum_k sum_{j!=k} m_k m_j/sqrt(r^2+eps^2)
+ * (NaN unless with_potential, which costs a second O(n^2) pass);  out[9..11] = sum m x / M;
+ * out[12] = steps taken;  out[13..15] = 0.  FP32 products, FP64 accumulation, fixed order.
+ * Synchronises the stream. */
+int colatus_diagnostics(double a, int with_potential, double out[16]);
+
+/* Copies the resident positions / velocities to host arrays float[n][4] (either may be
+ * NULL).  Synchronises the stream. */
+int colatus_download(float *pos_mass_host, float *vel_host);
+
+/* ---- instrumentation ------------------------------------------------------------------
+ * colatus_profile(1) makes the library bracket every force-kernel launch with CUDA events
+ * on the launching stream; colatus_profile_read synchronises and returns the number of
+ * bracketed launches and their summed duration in ms, then resets both.
+ * colatus_launch_count returns the number of kernels this library has launched. */
+int      colatus_profile(int enable);
+int      colatus_profile_read(double *total_ms, int64_t *launches);
+int64_t  colatus_launch_count(void);
+
+/* Geometry the force path picked for n bodies / target_count targets on this device:
+ * out[0] = targets per CTA, out[1] = target tiles, out[2] = source splits,
+ * out[3] = sources per split (padded), out[4] = CTAs per SM, out[5] = SM count,
+ * out[6] = kernel variant (targets per thread), out[7] = threads per CTA. */
+int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
+
+/* Tuning overrides for measurements (0 restores the automatic choice):
+ *   "targets_per_thread" in {0,1,2,4};  "source_splits" in [0,16]. */
+int colatus_set_option(const char *name, int64_t value);
+
+const char *colatus_last_error(void);
+
+/* ---- host-only cosmology, FP64 (eq. (2)) ---------------------------------- */
+typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosmo;
+
+/* H(a) = H0 sqrt(Om_R a^-4 + Om_M a^-3 + Om_K a^-2 + Om_L).  NaN if a <= 0. */
+double colatus_hubble(const colatus_cosmo *c, double a);
+/* a(t0 + dt) given a(t0) = a0, integrating da/dt = a H(a) (adaptive step doubling). */
+double colatus_a_advance(const colatus_cosmo *c, double a0, double dt);
+/* t(a) = integral_0^a da' / (a' H(a'));  +inf if it diverges (no matter, radiation or curvature). */
+double colatus_time_of_a(const colatus_cosmo *c, double a);
+/* integral_{t0}^{t0+dt} dt / a(t)^p with a(t0) = a0: drift (p=2) and kick (p=1) integrals of eq. (9). */
+double colatus_int_dt_over_a_pow(const colatus_cosmo *c, double a0, double dt, double p);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COLATUS_H */

@@ -1,0 +1,589 @@
+// colatus_api.cu -- the C-ABI boundary of libcolatus (include/colatus.h): argument validation,
+// launch geometry and kernel launches.  All arithmetic of the path lives in the kernels of
+// force_kernels.cuh / integrate_kernels.cuh; the host forms only the per-step coefficients.
+// Links the CUDA runtime only (no libtorch).  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+#include "../../include/colatus.h"
+#include "force_kernels.cuh"
+#include "integrate_kernels.cuh"
+
+namespace {
+
+using namespace colatus;
+
+constexpr int MAX_SPLITS = 16;        // source splits (partials kept in the workspace)
+constexpr int NSTAGES = 4;            // shared-memory ring depth
+constexpr int DIAG_BLOCKS_MAX = 1024;
+constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
+
+struct Geometry {
+    int I = 0, TJ = 0;
+    int64_t tiles_t = 0;
+    int splits = 0, tiles_per_split = 0;
+    int64_t n_pad = 0;   // sources covered = splits * tiles_per_split * TJ
+};
+
+struct Workspace {     // byte offsets inside the caller's workspace
+    size_t packed = 0, partials = 0, scratch_acc = 0, trace_slot = 0, diag = 0, stage_in = 0, stage_out = 0,
+           total = 0;
+};
+
+struct Context {
+    bool initialised = false;
+    double G = 0.0;
+    int device = 0, sm_count = 0, ctas_per_sm = 2;
+    unsigned char *ws = nullptr;
+    size_t ws_bytes = 0;
+    // resident state
+    bool uploaded = false;
+    float4 *pos = nullptr, *vel = nullptr, *acc = nullptr;
+    int64_t n = 0, t_begin = 0, t_count = 0;
+    float eps2 = 0.f;
+    cudaStream_t stream = nullptr;
+    int64_t step = 0;
+    // tracers
+    int trace_k = 0, trace_cap = 0;
+    float4 *ring = nullptr;
+    int64_t trace_n = 0;   // n for which the slot map was built
+    // instrumentation
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    int64_t launches = 0;
+    // tuning overrides (0 = automatic)
+    int force_I = 0, force_splits = 0;
+    char err[512] = "";
+};
+
+Context g;
+
+int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g.err, sizeof(g.err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(COLATUS_CUDA_ERROR, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                                        \
+    } while (0)
+
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+Workspace workspace_layout(int64_t n_max) {
+    Workspace w;
+    const size_t n = (size_t)n_max;
+    const size_t n_pad = round_up(n, (size_t)PAD_SOURCES) + (size_t)MAX_SPLITS * PAD_SOURCES;
+    size_t off = 0;
+    w.packed = off;      off += round_up(n_pad * 16, 256);
+    w.partials = off;    off += round_up((size_t)MAX_SPLITS * n * 16, 256);
+    w.scratch_acc = off; off += round_up(n * 16, 256);
+    w.trace_slot = off;  off += round_up(n * 4, 256);
+    w.diag = off;        off += round_up((size_t)(DIAG_BLOCKS_MAX + 2) * DIAG_Q * 8, 256);
+    w.stage_in = off;    off += round_up(n * 16, 256);
+    w.stage_out = off;   off += round_up(n * 16, 256);
+    w.total = off;
+    return w;
+}
+
+// Pick (I, TJ) and the source split so that CTAs ~ k * (SMs * CTAs/SM) with little padding
+// (DESIGN.md "Launch geometry").
+Geometry choose_geometry(int64_t n, int64_t t_count) {
+    static const int variants[3][2] = {{4, 1024}, {2, 512}, {1, 256}};
+    const int64_t slots = (int64_t)g.sm_count * g.ctas_per_sm;
+    Geometry best;
+    for (int v = 0; v < 3; ++v) {
+        const int I = variants[v][0], TJ = variants[v][1];
+        if (g.force_I && g.force_I != I) continue;
+        const int64_t tiles_t = (t_count + (int64_t)FORCE_THREADS * I - 1) / ((int64_t)FORCE_THREADS * I);
+        const int64_t src_tiles = (n + TJ - 1) / TJ;
+        const int64_t smax = src_tiles < MAX_SPLITS ? src_tiles : MAX_SPLITS;
+        if (!g.force_I && v < 2 && tiles_t * smax < slots) continue;   // too few CTAs: finer variant
+        double best_eff = -1.0;
+        for (int64_t s = 1; s <= smax; ++s) {
+            if (g.force_splits && s != g.force_splits && g.force_splits <= smax) continue;
+            const int64_t tps = (src_tiles + s - 1) / s;
+            const int64_t units = tiles_t * s;
+            const int64_t waves = (units + slots - 1) / slots;
+            double eff = (double)units / (double)(waves * slots) * (double)src_tiles / (double)(s * tps);
+            eff *= (double)tps / ((double)tps + 0.125);   // per-CTA prologue/epilogue
+            if (eff > best_eff * 1.002) {                 // prefer fewer splits on near ties
+                best_eff = eff;
+                best.I = I;
+                best.TJ = TJ;
+                best.tiles_t = tiles_t;
+                best.splits = (int)s;
+                best.tiles_per_split = (int)tps;
+                best.n_pad = s * tps * TJ;
+            }
+        }
+        break;
+    }
+    return best;
+}
+
+template <int I, int TJ, bool POT>
+cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
+                                 int64_t t_count, float eps2, float scale, int final_out, float4 *out,
+                                 int64_t out_stride, cudaStream_t st) {
+    auto kern = force_kernel<I, TJ, NSTAGES, POT, 2>;
+    const size_t smem = (size_t)NSTAGES * TJ * 16 + 2 * NSTAGES * sizeof(uint64_t);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    dim3 grid((unsigned)geo.tiles_t, (unsigned)geo.splits);
+    kern<<<grid, FORCE_THREADS, smem, st>>>(pos_mass, packed, t_begin, t_count, geo.tiles_per_split, eps2, scale,
+                                            final_out, out, out_stride);
+    return cudaGetLastError();
+}
+
+template <bool POT>
+cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
+                         int64_t t_count, float eps2, float scale, int final_out, float4 *out, int64_t out_stride,
+                         cudaStream_t st) {
+    switch (geo.I) {
+        case 4:
+            return launch_force_variant<4, 1024, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
+                                                      final_out, out, out_stride, st);
+        case 2:
+            return launch_force_variant<2, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
+                                                     final_out, out, out_stride, st);
+        default:
+            return launch_force_variant<1, 256, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
+                                                     final_out, out, out_stride, st);
+    }
+}
+
+// repack + force (+ reduce): the whole of step a3.  No validation here.
+int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2, float4 *out,
+               bool potential, cudaStream_t st) {
+    const Workspace w = workspace_layout(n);
+    if (w.total > g.ws_bytes)
+        return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
+                    (long long)n, w.total);
+    const Geometry geo = choose_geometry(n, t_count);
+    float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
+    float4 *partials = reinterpret_cast<float4 *>(g.ws + w.partials);
+
+    const int64_t pairs = geo.n_pad / 2;
+    repack_sources_kernel<<<(unsigned)((pairs + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+
+    const bool single = geo.splits == 1;
+    float4 *fout = single ? out : partials;
+    const float scale = single ? (float)g.G : 1.0f;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (g.profile) {
+        if (g.ev_used + 2 > g.ev_pool.size()) {
+            for (int i = 0; i < 64; ++i) {
+                cudaEvent_t e;
+                CUDA_TRY(cudaEventCreate(&e));
+                g.ev_pool.push_back(e);
+            }
+        }
+        e0 = g.ev_pool[g.ev_used++];
+        e1 = g.ev_pool[g.ev_used++];
+        CUDA_TRY(cudaEventRecord(e0, st));
+    }
+    cudaError_t e = potential ? launch_force<true>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single, fout,
+                                                   t_count, st)
+                              : launch_force<false>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single,
+                                                    fout, t_count, st);
+    CUDA_TRY(e);
+    g.launches++;
+    if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
+
+    if (!single) {
+        const unsigned blocks = (unsigned)((t_count + 255) / 256);
+        if (potential)
+            reduce_partials_kernel<true><<<blocks, 256, 0, st>>>(partials, t_count, geo.splits, t_count, (float)g.G,
+                                                                 eps2, pos_mass, t_begin, out);
+        else
+            reduce_partials_kernel<false><<<blocks, 256, 0, st>>>(partials, t_count, geo.splits, t_count,
+                                                                  (float)g.G, eps2, pos_mass, t_begin, out);
+        CUDA_TRY(cudaGetLastError());
+        g.launches++;
+    }
+    return COLATUS_OK;
+}
+
+int check_forces_args(const void *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2,
+                      const void *acc_out) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!pos_mass || !acc_out) return fail(COLATUS_INVALID_ARG, "null pointer");
+    if (n < 1 || n > 2147483647LL) return fail(COLATUS_INVALID_ARG, "n=%lld out of [1, 2^31-1]", (long long)n);
+    if (t_begin < 0 || t_count < 1 || t_begin + t_count > n)
+        return fail(COLATUS_INVALID_ARG, "target range [%lld, +%lld) outside [0, %lld)", (long long)t_begin,
+                    (long long)t_count, (long long)n);
+    if (!aligned16(pos_mass) || !aligned16(acc_out)) return fail(COLATUS_INVALID_ARG, "pointer not 16-byte aligned");
+    if (pos_mass == acc_out) return fail(COLATUS_INVALID_ARG, "pos_mass and acc_out alias");
+    if (!std::isfinite(eps2) || eps2 < 1e-30f) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-30");
+    return COLATUS_OK;
+}
+
+int enqueue_drift(double d) {
+    const unsigned blocks = (unsigned)((g.t_count + 255) / 256);
+    drift_kernel<<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, g.t_begin, g.t_count, (float)d);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
+int enqueue_force_kick_drift(double cv, double ck, double d2, float tag) {
+    int rc = run_forces(g.pos, g.n, g.t_begin, g.t_count, g.eps2, g.acc, false, g.stream);
+    if (rc) return rc;
+    const unsigned blocks = (unsigned)((g.t_count + 255) / 256);
+    if (g.trace_k > 0) {
+        const Workspace w = workspace_layout(g.n);
+        const int32_t *slot = reinterpret_cast<const int32_t *>(g.ws + w.trace_slot);
+        float4 *row = g.ring + (size_t)(g.step % g.trace_cap) * g.trace_k;
+        kick_drift_kernel<true><<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, (float)cv,
+                                                              (float)ck, (float)d2, slot, row, tag);
+    } else {
+        kick_drift_kernel<false><<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, (float)cv,
+                                                               (float)ck, (float)d2, nullptr, nullptr, tag);
+    }
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    g.step++;
+    return COLATUS_OK;
+}
+
+int build_trace_map(const int32_t *idx_dev) {
+    const Workspace w = workspace_layout(g.n);
+    if (w.total > g.ws_bytes) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace too small for n=%lld", (long long)g.n);
+    int32_t *slot = reinterpret_cast<int32_t *>(g.ws + w.trace_slot);
+    trace_fill_kernel<<<(unsigned)((g.n + 255) / 256), 256, 0, g.stream>>>(slot, g.n);
+    CUDA_TRY(cudaGetLastError());
+    trace_scatter_kernel<<<(unsigned)((g.trace_k + 255) / 256), 256, 0, g.stream>>>(slot, g.n, idx_dev, g.trace_k);
+    CUDA_TRY(cudaGetLastError());
+    g.launches += 2;
+    return COLATUS_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+size_t colatus_workspace_bytes(int64_t n_max) {
+    if (n_max < 1) return 0;
+    return workspace_layout(n_max).total;
+}
+
+int colatus_init(const colatus_config *cfg) {
+    if (g.initialised) return fail(COLATUS_ALREADY_INITIALISED, "colatus_init called twice without colatus_shutdown");
+    if (!cfg) return fail(COLATUS_INVALID_ARG, "cfg is null");
+    if (!std::isfinite(cfg->G)) return fail(COLATUS_INVALID_ARG, "G is not finite");
+    if (!cfg->workspace_dev || (reinterpret_cast<uintptr_t>(cfg->workspace_dev) & 255u))
+        return fail(COLATUS_INVALID_ARG, "workspace_dev is null or not 256-byte aligned");
+    CUDA_TRY(cudaSetDevice(cfg->device));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, cfg->device));
+    if (prop.major != 10)
+        return fail(COLATUS_UNSUPPORTED_DEVICE, "device %d (%s) is cc %d.%d; libcolatus is built for sm_100a only",
+                    cfg->device, prop.name, prop.major, prop.minor);
+    g.G = cfg->G;
+    g.device = cfg->device;
+    g.sm_count = prop.multiProcessorCount;
+    g.ctas_per_sm = 2;
+    g.ws = static_cast<unsigned char *>(cfg->workspace_dev);
+    g.ws_bytes = cfg->workspace_bytes;
+    g.uploaded = false;
+    g.trace_k = 0;
+    g.step = 0;
+    g.profile = false;
+    g.ev_used = 0;
+    g.force_I = g.force_splits = 0;
+    g.initialised = true;
+    g.err[0] = 0;
+    return COLATUS_OK;
+}
+
+void colatus_shutdown(void) {
+    for (cudaEvent_t e : g.ev_pool) cudaEventDestroy(e);
+    g.ev_pool.clear();
+    g.ev_used = 0;
+    g.initialised = false;
+    g.uploaded = false;
+    g.trace_k = 0;
+    g.ws = nullptr;
+    g.ws_bytes = 0;
+}
+
+int colatus_forces(const void *pos_mass_dev, int64_t n, float eps2, void *acc_out_dev, void *cuda_stream) {
+    int rc = check_forces_args(pos_mass_dev, n, 0, n, eps2, acc_out_dev);
+    if (rc) return rc;
+    return run_forces(static_cast<const float4 *>(pos_mass_dev), n, 0, n, eps2, static_cast<float4 *>(acc_out_dev),
+                      false, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int colatus_forces_potential(const void *pos_mass_dev, int64_t n, float eps2, void *acc_out_dev, void *cuda_stream) {
+    int rc = check_forces_args(pos_mass_dev, n, 0, n, eps2, acc_out_dev);
+    if (rc) return rc;
+    return run_forces(static_cast<const float4 *>(pos_mass_dev), n, 0, n, eps2, static_cast<float4 *>(acc_out_dev),
+                      true, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int colatus_forces_range(const void *pos_mass_dev, int64_t n, int64_t target_begin, int64_t target_count, float eps2,
+                         void *acc_out_dev, void *cuda_stream) {
+    int rc = check_forces_args(pos_mass_dev, n, target_begin, target_count, eps2, acc_out_dev);
+    if (rc) return rc;
+    return run_forces(static_cast<const float4 *>(pos_mass_dev), n, target_begin, target_count, eps2,
+                      static_cast<float4 *>(acc_out_dev), false, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int colatus_forces_host(const float *pos_mass_host, int64_t n, float eps2, float *acc_out_host, void *cuda_stream) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!pos_mass_host || !acc_out_host) return fail(COLATUS_INVALID_ARG, "null pointer");
+    if (n < 1 || n > 2147483647LL) return fail(COLATUS_INVALID_ARG, "n=%lld out of [1, 2^31-1]", (long long)n);
+    if (!std::isfinite(eps2) || eps2 < 1e-30f) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-30");
+    const Workspace w = workspace_layout(n);
+    if (w.total > g.ws_bytes)
+        return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
+                    (long long)n, w.total);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    float4 *din = reinterpret_cast<float4 *>(g.ws + w.stage_in);
+    float4 *dout = reinterpret_cast<float4 *>(g.ws + w.stage_out);
+    CUDA_TRY(cudaMemcpyAsync(din, pos_mass_host, (size_t)n * 16, cudaMemcpyHostToDevice, st));
+    int rc = run_forces(din, n, 0, n, eps2, dout, false, st);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(acc_out_host, dout, (size_t)n * 16, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return COLATUS_OK;
+}
+
+int colatus_upload(void *pos_mass_dev, void *vel_dev, void *acc_dev, int64_t n, float eps2, void *cuda_stream) {
+    int rc = check_forces_args(pos_mass_dev, n, 0, n, eps2, acc_dev);
+    if (rc) return rc;
+    if (!vel_dev || !aligned16(vel_dev)) return fail(COLATUS_INVALID_ARG, "vel_dev null or misaligned");
+    if (vel_dev == pos_mass_dev || vel_dev == acc_dev) return fail(COLATUS_INVALID_ARG, "state buffers alias");
+    if (workspace_layout(n).total > g.ws_bytes)
+        return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
+                    (long long)n, workspace_layout(n).total);
+    g.pos = static_cast<float4 *>(pos_mass_dev);
+    g.vel = static_cast<float4 *>(vel_dev);
+    g.acc = static_cast<float4 *>(acc_dev);
+    g.n = n;
+    g.t_begin = 0;
+    g.t_count = n;
+    g.eps2 = eps2;
+    g.stream = static_cast<cudaStream_t>(cuda_stream);
+    g.step = 0;
+    g.trace_k = 0;
+    g.uploaded = true;
+    return COLATUS_OK;
+}
+
+int colatus_set_target_range(int64_t target_begin, int64_t target_count) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (target_begin < 0 || target_count < 1 || target_begin + target_count > g.n)
+        return fail(COLATUS_INVALID_ARG, "target range outside [0, n)");
+    g.t_begin = target_begin;
+    g.t_count = target_count;
+    return COLATUS_OK;
+}
+
+int colatus_step_coeffs(double d1, double cv, double ck, double d2) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!std::isfinite(d1) || !std::isfinite(cv) || !std::isfinite(ck) || !std::isfinite(d2))
+        return fail(COLATUS_INVALID_ARG, "non-finite step coefficient");
+    int rc = enqueue_drift(d1);
+    if (rc) return rc;
+    return enqueue_force_kick_drift(cv, ck, d2, 0.f);
+}
+
+int colatus_step(double tau, double a, double H) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!std::isfinite(tau) || !std::isfinite(a) || !std::isfinite(H))
+        return fail(COLATUS_INVALID_ARG, "non-finite tau, a or H");
+    if (!(a > 0.0)) return fail(COLATUS_INVALID_ARG, "a must be > 0");
+    if (!(1.0 + H * tau > 0.0)) return fail(COLATUS_INVALID_ARG, "1 + H tau must be > 0");
+    // eq. (4): drag factor and kick coefficient, in double
+    const double cv = (1.0 - H * tau) / (1.0 + H * tau);
+    const double ck = tau / (a * a * a * (1.0 + H * tau));
+    int rc = enqueue_drift(0.5 * tau);                                   // eq. (3)
+    if (rc) return rc;
+    return enqueue_force_kick_drift(cv, ck, 0.5 * tau, (float)a);       // eqs. (1), (4), (5)
+}
+
+int colatus_drift(double d) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!std::isfinite(d)) return fail(COLATUS_INVALID_ARG, "non-finite drift coefficient");
+    return enqueue_drift(d);
+}
+
+int colatus_force_kick_drift(double cv, double ck, double d2) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!std::isfinite(cv) || !std::isfinite(ck) || !std::isfinite(d2))
+        return fail(COLATUS_INVALID_ARG, "non-finite step coefficient");
+    return enqueue_force_kick_drift(cv, ck, d2, 0.f);
+}
+
+int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_steps) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (k < 0) return fail(COLATUS_INVALID_ARG, "k < 0");
+    if (k == 0) {
+        g.trace_k = 0;
+        return COLATUS_OK;
+    }
+    if (!idx_dev || !ring_dev || !aligned16(ring_dev)) return fail(COLATUS_INVALID_ARG, "null or misaligned pointer");
+    if (capacity_steps < 1) return fail(COLATUS_INVALID_ARG, "capacity_steps < 1");
+    g.trace_k = k;
+    g.trace_cap = capacity_steps;
+    g.ring = static_cast<float4 *>(ring_dev);
+    int rc = build_trace_map(idx_dev);
+    if (rc) g.trace_k = 0;
+    return rc;
+}
+
+int colatus_trace_read(float *host_out, int64_t first_step, int n_steps) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded || g.trace_k == 0) return fail(COLATUS_NOT_UPLOADED, "no tracers configured");
+    if (!host_out || n_steps < 1 || first_step < 0) return fail(COLATUS_INVALID_ARG, "bad arguments");
+    if (first_step + n_steps > g.step || first_step < g.step - g.trace_cap)
+        return fail(COLATUS_INVALID_ARG, "steps [%lld, +%d) not held by the ring (step=%lld, capacity=%d)",
+                    (long long)first_step, n_steps, (long long)g.step, g.trace_cap);
+    const size_t row = (size_t)g.trace_k * 16;
+    for (int s = 0; s < n_steps;) {   // contiguous runs of ring rows
+        const int64_t slot = (first_step + s) % g.trace_cap;
+        int run = n_steps - s;
+        if (slot + run > g.trace_cap) run = (int)(g.trace_cap - slot);
+        CUDA_TRY(cudaMemcpyAsync(reinterpret_cast<unsigned char *>(host_out) + (size_t)s * row,
+                                 reinterpret_cast<unsigned char *>(g.ring) + (size_t)slot * row, (size_t)run * row,
+                                 cudaMemcpyDeviceToHost, g.stream));
+        s += run;
+    }
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    return COLATUS_OK;
+}
+
+int colatus_diagnostics(double a, int with_potential, double out[16]) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!out) return fail(COLATUS_INVALID_ARG, "out is null");
+    if (!std::isfinite(a) || !(a > 0.0)) return fail(COLATUS_INVALID_ARG, "a must be finite and > 0");
+    const Workspace w = workspace_layout(g.n);
+    float4 *scratch = reinterpret_cast<float4 *>(g.ws + w.scratch_acc);
+    double *partial = reinterpret_cast<double *>(g.ws + w.diag);
+    if (with_potential) {
+        int rc = run_forces(g.pos, g.n, 0, g.n, g.eps2, scratch, true, g.stream);
+        if (rc) return rc;
+    }
+    int blocks = (int)((g.n + 255) / 256);
+    if (blocks > DIAG_BLOCKS_MAX) blocks = DIAG_BLOCKS_MAX;
+    diagnostics_partial_kernel<<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, with_potential ? scratch : nullptr, g.n,
+                                                             partial);
+    CUDA_TRY(cudaGetLastError());
+    double *final_dev = partial + (size_t)DIAG_BLOCKS_MAX * DIAG_Q;
+    diagnostics_final_kernel<<<1, 32, 0, g.stream>>>(partial, blocks, final_dev);
+    CUDA_TRY(cudaGetLastError());
+    g.launches += 2;
+    double q[DIAG_Q];
+    CUDA_TRY(cudaMemcpyAsync(q, final_dev, sizeof(q), cudaMemcpyDeviceToHost, g.stream));
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    out[0] = q[0];
+    for (int c = 0; c < 3; ++c) {
+        out[1 + c] = q[1 + c];
+        out[4 + c] = a * a * q[1 + c];
+        out[9 + c] = q[5 + c] / q[0];
+    }
+    out[7] = 0.5 * a * a * q[4];
+    out[8] = with_potential ? 0.5 * q[8] / a : std::numeric_limits<double>::quiet_NaN();
+    out[12] = (double)g.step;
+    out[13] = out[14] = out[15] = 0.0;
+    return COLATUS_OK;
+}
+
+int colatus_download(float *pos_mass_host, float *vel_host) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (pos_mass_host)
+        CUDA_TRY(cudaMemcpyAsync(pos_mass_host, g.pos, (size_t)g.n * 16, cudaMemcpyDeviceToHost, g.stream));
+    if (vel_host) CUDA_TRY(cudaMemcpyAsync(vel_host, g.vel, (size_t)g.n * 16, cudaMemcpyDeviceToHost, g.stream));
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    return COLATUS_OK;
+}
+
+int colatus_profile(int enable) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    g.profile = enable != 0;
+    g.ev_used = 0;
+    return COLATUS_OK;
+}
+
+int colatus_profile_read(double *total_ms, int64_t *launches) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!total_ms || !launches) return fail(COLATUS_INVALID_ARG, "null pointer");
+    double sum = 0.0;
+    for (size_t i = 0; i + 1 < g.ev_used; i += 2) {
+        CUDA_TRY(cudaEventSynchronize(g.ev_pool[i + 1]));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, g.ev_pool[i], g.ev_pool[i + 1]));
+        sum += ms;
+    }
+    *total_ms = sum;
+    *launches = (int64_t)(g.ev_used / 2);
+    g.ev_used = 0;
+    return COLATUS_OK;
+}
+
+int64_t colatus_launch_count(void) { return g.launches; }
+
+int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!out || n < 1 || target_count < 1 || target_count > n) return fail(COLATUS_INVALID_ARG, "bad arguments");
+    const Geometry geo = choose_geometry(n, target_count);
+    out[0] = (int64_t)FORCE_THREADS * geo.I;
+    out[1] = geo.tiles_t;
+    out[2] = geo.splits;
+    out[3] = (int64_t)geo.tiles_per_split * geo.TJ;
+    out[4] = g.ctas_per_sm;
+    out[5] = g.sm_count;
+    out[6] = geo.I;
+    out[7] = FORCE_THREADS;
+    return COLATUS_OK;
+}
+
+int colatus_set_option(const char *name, int64_t value) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!name) return fail(COLATUS_INVALID_ARG, "name is null");
+    if (!strcmp(name, "targets_per_thread")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4) return fail(COLATUS_INVALID_ARG, "must be 0,1,2,4");
+        g.force_I = (int)value;
+    } else if (!strcmp(name, "source_splits")) {
+        if (value < 0 || value > MAX_SPLITS) return fail(COLATUS_INVALID_ARG, "must be in [0, %d]", MAX_SPLITS);
+        g.force_splits = (int)value;
+    } else {
+        return fail(COLATUS_INVALID_ARG, "unknown option %s", name);
+    }
+    return COLATUS_OK;
+}
+
+const char *colatus_last_error(void) { return g.err; }
+
+}  // extern "C"

@@ -1,0 +1,125 @@
+// integrate_kernels.cuh -- eqs. (3)-(5) of arXiv 1208.3444 and the tracer record.
+//
+//   x^{n+1/2} = x^n + (tau/2) v^n                                                     (3)  drift_kernel
+//   v^{n+1}   = v^n (1-H tau)/(1+H tau) + F tau/(a^3 (1+H tau))                       (4)  kick_drift_kernel
+//   x^{n+1}   = x^{n+1/2} + (tau/2) v^{n+1}                                           (5)  (same kernel)
+//
+// The coefficients d1 = tau/2, cv = (1-H tau)/(1+H tau), ck = tau/(a^3 (1+H tau)), d2 = tau/2 are
+// formed in double on the host.  Elementwise, HBM-bound: one float4 per array per body, coalesced.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace colatus {
+
+// eq. (3): x += d v   (mass in .w untouched)
+__global__ void __launch_bounds__(256) drift_kernel(float4 *__restrict__ pos_mass, const float4 *__restrict__ vel,
+                                                    int64_t begin, int64_t count, float d) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    float4 p = pos_mass[begin + i];
+    const float4 v = vel[begin + i];
+    p.x = fmaf(d, v.x, p.x);
+    p.y = fmaf(d, v.y, p.y);
+    p.z = fmaf(d, v.z, p.z);
+    pos_mass[begin + i] = p;
+}
+
+// eqs. (4)+(5) fused, plus the tracer record: acc is indexed from 0 for the
+// target range.  trace_slot[k] >= 0 marks particle k as tracer number trace_slot[k]; its v^{n+1}
+// goes to ring_row[slot] = (vx, vy, vz, tag).
+template <bool TRACE>
+__global__ void __launch_bounds__(256)
+kick_drift_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, const float4 *__restrict__ acc,
+                  int64_t begin, int64_t count, float cv, float ck, float d2,
+                  const int32_t *__restrict__ trace_slot, float4 *__restrict__ ring_row, float tag) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    float4 p = pos_mass[begin + i];
+    float4 v = vel[begin + i];
+    const float4 f = acc[i];
+    v.x = fmaf(ck, f.x, cv * v.x);
+    v.y = fmaf(ck, f.y, cv * v.y);
+    v.z = fmaf(ck, f.z, cv * v.z);
+    p.x = fmaf(d2, v.x, p.x);
+    p.y = fmaf(d2, v.y, p.y);
+    p.z = fmaf(d2, v.z, p.z);
+    vel[begin + i] = v;
+    pos_mass[begin + i] = p;
+    if (TRACE) {
+        const int32_t s = trace_slot[begin + i];
+        if (s >= 0) ring_row[s] = make_float4(v.x, v.y, v.z, tag);
+    }
+}
+
+// tracer slot map: slot[k] = t if idx[t] == k else -1
+__global__ void __launch_bounds__(256) trace_fill_kernel(int32_t *__restrict__ slot, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) slot[i] = -1;
+}
+__global__ void __launch_bounds__(256)
+trace_scatter_kernel(int32_t *__restrict__ slot, int64_t n, const int32_t *__restrict__ idx, int k) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < k) {
+        const int32_t j = idx[t];
+        if (j >= 0 && (int64_t)j < n) slot[j] = t;
+    }
+}
+
+// ---- diagnostics (eq. (7)): FP64 accumulation, fixed order ---------------------------
+// per-block partial q[0..8] = sum m, sum m vx, sum m vy, sum m vz, sum m v^2, sum m x, sum m y, sum m z,
+// sum m phi (phi = acc.w of a potential pass, or 0).
+constexpr int DIAG_Q = 9;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(256) diagnostics_partial_kernel(const float4 *__restrict__ pos_mass,
+                                                                  const float4 *__restrict__ vel,
+                                                                  const float4 *__restrict__ phi_w, int64_t n,
+                                                                  double *__restrict__ partial) {
+    double q[DIAG_Q];
+#pragma unroll
+    for (int c = 0; c < DIAG_Q; ++c) q[c] = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float4 p = pos_mass[i];
+        const float4 v = vel[i];
+        const double m = p.w;
+        q[0] += m;
+        q[1] += m * v.x;
+        q[2] += m * v.y;
+        q[3] += m * v.z;
+        q[4] += m * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+        q[5] += m * p.x;
+        q[6] += m * p.y;
+        q[7] += m * p.z;
+        if (phi_w) q[8] += m * phi_w[i].w;
+    }
+    __shared__ double sh[8][DIAG_Q];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int c = 0; c < DIAG_Q; ++c) {
+        const double s = warp_sum(q[c]);
+        if (lane == 0) sh[warp][c] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < DIAG_Q) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += sh[w][threadIdx.x];
+        partial[(size_t)blockIdx.x * DIAG_Q + threadIdx.x] = s;
+    }
+}
+
+__global__ void diagnostics_final_kernel(const double *__restrict__ partial, int blocks, double *__restrict__ out) {
+    const int c = threadIdx.x;
+    if (c < DIAG_Q) {
+        double s = 0.0;
+        for (int b = 0; b < blocks; ++b) s += partial[(size_t)b * DIAG_Q + c];
+        out[c] = s;
+    }
+}
+
+}  // namespace colatus

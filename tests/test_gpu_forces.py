@@ -1,0 +1,170 @@
+"""T2 (forces): the CUDA path of eq. (1) against the FP64 oracle, through the C ABI.
+
+Tolerances are north_star's (readings G17): over the checked targets
+    median_k |a_gpu - a_ref| / |a_ref|  <= 1e-5      and
+    max_k |a_gpu - a_ref| / rms_k |a_ref| <= 1e-4.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+from paper_1208_3444_b200 import binding as B  # noqa: E402
+from paper_1208_3444_b200 import inputs  # noqa: E402
+
+MEDIAN_TOL = 1e-5
+MAX_TOL = 1e-4
+
+
+def force_errors(acc_gpu, acc_ref):
+    d = np.linalg.norm(acc_gpu.astype(np.float64) - acc_ref, axis=1)
+    nr = np.linalg.norm(acc_ref, axis=1)
+    return float(np.median(d / nr)), float(d.max() / np.sqrt((nr ** 2).mean()))
+
+
+@pytest.fixture(scope="module")
+def session():
+    from paper_1208_3444_b200.harness import Session
+    s = Session(1.0, 1 << 22)
+    yield s
+    s.close()
+
+
+def _check_config(session, index, n_targets=None):
+    cfg, pm, _ = inputs.make_config(index)
+    tg = inputs.sample_targets(cfg, n_targets)
+    # G is fixed at init (1.0); F is linear in G, so compare at G=1 on both sides
+    acc = session.forces(pm, cfg.eps2).cpu().numpy()
+    assert np.all(acc[:, 3] == 0.0)
+    ref = oracle.forces(pm, cfg.eps2, 1.0, tg)
+    med, mx = force_errors(acc[tg, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (index, med, mx)
+    # Newton's third law on the GPU result (P2): |sum m F| / sum m |F|
+    m = pm[:, 3].astype(np.float64)
+    F = acc[:, :3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * F).sum(0)) / (m * np.linalg.norm(F, axis=1)).sum() < 2e-6
+    return med, mx
+
+
+def test_forces_config1_all_targets(session):
+    _check_config(session, 1)
+
+
+def test_forces_config2_all_targets(session):
+    _check_config(session, 2)
+
+
+def test_forces_config3_sampled_targets(session):
+    # all 131072 targets take the oracle ~15 s on 8 cores; 16384 seeded targets keep the suite short
+    _check_config(session, 3, n_targets=16384)
+
+
+def test_forces_config4_full_size_sampled(session):
+    """N = 2^20 in the launch configuration bench.py times; 4096 seeded targets (BASELINE config 4)."""
+    geo = B.colatus_force_geometry(1 << 20)
+    assert geo["targets_per_thread"] == 4
+    _check_config(session, 4)
+
+
+def test_forces_config5_full_size_sampled(session):
+    """N = 2^22; 4096 seeded targets (BASELINE config 5)."""
+    _check_config(session, 5)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 255, 256, 257, 1000, 1025, 4099, 9001])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4])
+def test_forces_ragged_sizes_all_variants(session, n, variant):
+    """Ragged tails, sizes below one tile, every kernel variant, potential included."""
+    rng = np.random.Generator(np.random.PCG64(100 + n))
+    pm = np.empty((n, 4), dtype=np.float32)
+    pm[:, :3] = rng.random((n, 3))
+    pm[:, 3] = (rng.random(n) + 0.5) / n
+    eps2 = np.float32(0.02 ** 2)
+    B.colatus_set_option("targets_per_thread", variant)
+    try:
+        out = session.forces(pm, eps2, potential=True).cpu().numpy()
+    finally:
+        B.colatus_set_option("targets_per_thread", 0)
+    ref, phi = oracle.forces(pm, eps2, 1.0, potential=True)
+    if n == 1:
+        assert np.all(out[:, :3] == 0.0) and abs(out[0, 3]) < 1e-6 * pm[0, 3] / 0.02
+        return
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (n, variant, med, mx)
+    assert np.allclose(out[:, 3], phi, rtol=2e-5, atol=0)
+
+
+@pytest.mark.parametrize("splits", [1, 2, 3, 5, 16])
+def test_forces_source_splits(session, splits):
+    cfg, pm, _ = inputs.make_config(3, n_override=20000)
+    B.colatus_set_option("source_splits", splits)
+    try:
+        out = session.forces(pm, cfg.eps2).cpu().numpy()
+    finally:
+        B.colatus_set_option("source_splits", 0)
+    ref = oracle.forces(pm, cfg.eps2, 1.0)
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (splits, med, mx)
+
+
+def test_forces_range_matches_full(session):
+    cfg, pm, _ = inputs.make_config(1)
+    full = session.forces(pm, cfg.eps2).cpu().numpy()
+    for b, c in ((0, 4096), (0, 1), (4095, 1), (1000, 2049), (123, 3000)):
+        part = session.forces(pm, cfg.eps2, target_range=(b, c)).cpu().numpy()
+        ref = oracle.forces(pm, cfg.eps2, 1.0, np.arange(b, b + c))
+        med, mx = force_errors(part[:, :3], ref)
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL
+        # same arithmetic per target, whatever the tiling of the target axis
+        assert np.allclose(part[:, :3], full[b:b + c, :3], rtol=2e-6, atol=1e-7)
+
+
+def test_forces_host_entry_point(session):
+    cfg, pm, _ = inputs.make_config(1)
+    out = np.full((cfg.n, 4), np.nan, dtype=np.float32)
+    B.colatus_forces_host(pm, cfg.n, cfg.eps2, out)
+    dev = session.forces(pm, cfg.eps2).cpu().numpy()
+    assert np.array_equal(out, dev)
+
+
+def test_forces_bitwise_reproducible(session):
+    cfg, pm, _ = inputs.make_config(2)
+    a = session.forces(pm, cfg.eps2).cpu().numpy()
+    b = session.forces(pm, cfg.eps2).cpu().numpy()
+    assert np.array_equal(a, b)
+
+
+def test_forces_degenerate_inputs(session):
+    """Coincident distinct particles contribute 0 to each other (G4); zero-mass sources contribute 0."""
+    rng = np.random.Generator(np.random.PCG64(7))
+    n = 600
+    pm = np.empty((n, 4), dtype=np.float32)
+    pm[:, :3] = rng.random((n, 3))
+    pm[:, 3] = 1.0 / n
+    pm[1, :3] = pm[0, :3]
+    pm[5, 3] = 0.0
+    eps2 = np.float32(1e-4)
+    out = session.forces(pm, eps2).cpu().numpy()
+    ref = oracle.forces(pm, eps2, 1.0)
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL
+    without = np.delete(pm, 5, axis=0)
+    out2 = session.forces(without, eps2).cpu().numpy()
+    assert np.allclose(np.delete(out, 5, axis=0)[:, :3], out2[:, :3], rtol=1e-5, atol=1e-6)
+
+
+def test_closed_form_three_body_on_gpu(session, golden_dir):
+    """The exact rational example of tests/golden/three_body_rational.txt, straight through the ABI."""
+    import os
+    from fractions import Fraction
+    pm = np.array([[0, 0, 0, 1], [1, 2, 2, 2], [2, 4, 0, 3]], dtype=np.float32)
+    out = session.forces(pm, np.float32(16.0)).cpu().numpy()
+    rows = {}
+    with open(os.path.join(golden_dir, "three_body_rational.txt")) as fh:
+        for line in fh:
+            if not line.startswith("#") and line.strip():
+                t = line.split()
+                rows[t[0]] = [float(Fraction(s)) for s in t[1:]]
+    for i, body in enumerate("ABC"):
+        assert np.allclose(out[i, :3], rows[body], rtol=2e-6, atol=1e-8)
