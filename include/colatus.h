@@ -116,6 +116,11 @@ int colatus_upload(void *pos_mass_dev, void *vel_dev, void *acc_dev, int64_t n, 
  * a > 0 and 1 + H tau > 0.  Asynchronous. */
 int colatus_step(double tau, double a, double H);
 
+/* The four coefficients colatus_step uses, formed in double from eqs. (3)-(5):
+ * out = { d1 = tau/2, cv = (1-H tau)/(1+H tau), ck = tau/(a^3 (1+H tau)), d2 = tau/2 }.
+ * Host only; same argument checks as colatus_step. */
+int colatus_step_coefficients(double tau, double a, double H, double out[4]);
+
 /* Generic drift-kick-drift:  x += d1 v;  F = eq.(1)(x);  v = cv v + ck F;  x += d2 v.
  * Covers the symplectic operators of eq. (9), with v standing for p/m.
  * Asynchronous. */
@@ -146,11 +151,12 @@ int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_st
 int colatus_trace_read(float *host_out, int64_t first_step, int n_steps);
 
 /* ---- diagnostics (eq. (7)) ------------------------------
+ * Sums over the resident target range (all n bodies unless colatus_set_target_range):
  * out[0] = M = sum m;  out[1..3] = P = sum m v;  out[4..6] = a^2 P;
  * out[7] = T = 1/2 sum m a^2 v^2;  out[8] = W = -(G/2a) sum_k sum_{j!=k} m_k m_j/sqrt(r^2+eps^2)
- * (NaN unless with_potential, which costs a second O(n^2) pass);  out[9..11] = sum m x / M;
- * out[12] = steps taken;  out[13..15] = 0.  FP32 products, FP64 accumulation, fixed order.
- * Synchronises the stream. */
+ * with k over the range and j over all n (NaN unless with_potential, which costs a second
+ * O(n^2) pass);  out[9..11] = sum m x / M;  out[12] = steps taken;  out[13..15] = sum m x
+ * (so that shards can be added).  FP64 accumulation in a fixed order.  Synchronises the stream. */
 int colatus_diagnostics(double a, int with_potential, double out[16]);
 
 /* Copies the resident positions / velocities to host arrays float[n][4] (either may be

@@ -50,6 +50,7 @@ SIGNATURES = {
     "colatus_forces_host": (c_int, [c_void_p, c_int64, c_float, c_void_p, c_void_p]),
     "colatus_upload": (c_int, [c_void_p, c_void_p, c_void_p, c_int64, c_float, c_void_p]),
     "colatus_step": (c_int, [c_double, c_double, c_double]),
+    "colatus_step_coefficients": (c_int, [c_double, c_double, c_double, POINTER(c_double)]),
     "colatus_step_coeffs": (c_int, [c_double, c_double, c_double, c_double]),
     "colatus_set_target_range": (c_int, [c_int64, c_int64]),
     "colatus_drift": (c_int, [c_double]),
@@ -175,6 +176,12 @@ def colatus_upload(pos_mass, vel, acc, n, eps2, stream=None):
 
 def colatus_step(tau, a, H):
     _check(lib().colatus_step(float(tau), float(a), float(H)))
+
+
+def colatus_step_coefficients(tau, a, H):
+    out = (c_double * 4)()
+    _check(lib().colatus_step_coefficients(float(tau), float(a), float(H), out))
+    return tuple(out)
 
 
 def colatus_step_coeffs(d1, cv, ck, d2):

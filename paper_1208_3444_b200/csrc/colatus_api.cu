@@ -413,19 +413,28 @@ int colatus_step_coeffs(double d1, double cv, double ck, double d2) {
     return enqueue_force_kick_drift(cv, ck, d2, 0.f);
 }
 
-int colatus_step(double tau, double a, double H) {
-    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
-    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+int colatus_step_coefficients(double tau, double a, double H, double out[4]) {
+    if (!out) return fail(COLATUS_INVALID_ARG, "out is null");
     if (!std::isfinite(tau) || !std::isfinite(a) || !std::isfinite(H))
         return fail(COLATUS_INVALID_ARG, "non-finite tau, a or H");
     if (!(a > 0.0)) return fail(COLATUS_INVALID_ARG, "a must be > 0");
     if (!(1.0 + H * tau > 0.0)) return fail(COLATUS_INVALID_ARG, "1 + H tau must be > 0");
-    // eq. (4): drag factor and kick coefficient, in double
-    const double cv = (1.0 - H * tau) / (1.0 + H * tau);
-    const double ck = tau / (a * a * a * (1.0 + H * tau));
-    int rc = enqueue_drift(0.5 * tau);                                   // eq. (3)
+    out[0] = 0.5 * tau;                                   // eq. (3)
+    out[1] = (1.0 - H * tau) / (1.0 + H * tau);           // eq. (4): drag factor
+    out[2] = tau / (a * a * a * (1.0 + H * tau));         // eq. (4): kick coefficient (a^-3 applied here, G5)
+    out[3] = 0.5 * tau;                                   // eq. (5)
+    return COLATUS_OK;
+}
+
+int colatus_step(double tau, double a, double H) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    double c[4];
+    int rc = colatus_step_coefficients(tau, a, H, c);
     if (rc) return rc;
-    return enqueue_force_kick_drift(cv, ck, 0.5 * tau, (float)a);       // eqs. (1), (4), (5)
+    rc = enqueue_drift(c[0]);                                            // eq. (3)
+    if (rc) return rc;
+    return enqueue_force_kick_drift(c[1], c[2], c[3], (float)a);         // eqs. (1), (4), (5)
 }
 
 int colatus_drift(double d) {
@@ -491,13 +500,13 @@ int colatus_diagnostics(double a, int with_potential, double out[16]) {
     float4 *scratch = reinterpret_cast<float4 *>(g.ws + w.scratch_acc);
     double *partial = reinterpret_cast<double *>(g.ws + w.diag);
     if (with_potential) {
-        int rc = run_forces(g.pos, g.n, 0, g.n, g.eps2, scratch, true, g.stream);
+        int rc = run_forces(g.pos, g.n, g.t_begin, g.t_count, g.eps2, scratch, true, g.stream);
         if (rc) return rc;
     }
-    int blocks = (int)((g.n + 255) / 256);
+    int blocks = (int)((g.t_count + 255) / 256);
     if (blocks > DIAG_BLOCKS_MAX) blocks = DIAG_BLOCKS_MAX;
-    diagnostics_partial_kernel<<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, with_potential ? scratch : nullptr, g.n,
-                                                             partial);
+    diagnostics_partial_kernel<<<blocks, 256, 0, g.stream>>>(g.pos + g.t_begin, g.vel + g.t_begin,
+                                                             with_potential ? scratch : nullptr, g.t_count, partial);
     CUDA_TRY(cudaGetLastError());
     double *final_dev = partial + (size_t)DIAG_BLOCKS_MAX * DIAG_Q;
     diagnostics_final_kernel<<<1, 32, 0, g.stream>>>(partial, blocks, final_dev);
@@ -515,7 +524,7 @@ int colatus_diagnostics(double a, int with_potential, double out[16]) {
     out[7] = 0.5 * a * a * q[4];
     out[8] = with_potential ? 0.5 * q[8] / a : std::numeric_limits<double>::quiet_NaN();
     out[12] = (double)g.step;
-    out[13] = out[14] = out[15] = 0.0;
+    for (int c = 0; c < 3; ++c) out[13 + c] = q[5 + c];
     return COLATUS_OK;
 }
 
