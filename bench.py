@@ -38,7 +38,7 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-kernel launch at N = 2^20 from the
 # `ncu --set full` capture summarised in profiles/ (None until that capture exists).
-FORCE_KERNEL_DRAM_TRAFFIC_BYTES = 231209728     # profiles/r01_force_kernel_ncu_full.txt
+FORCE_KERNEL_DRAM_TRAFFIC_BYTES = 133545728     # profiles/r01_force_kernel_ncu_full.txt
 METRIC = "Ginteractions/s softened direct-sum gravity at N=2^20; % of FP32 FMA peak"
 UNIT = "Ginteractions/s"
 BENCH_TAU = 1.0e-6                         # step size of the bench steps (EdS background from a = 0.02)
@@ -234,11 +234,14 @@ def run_native(args):
 
     # ---- roofline of the dominant kernel (force kernel), from events inside the timed region
     pairs_per_launch = float(count) * n
+    geo = B.colatus_force_geometry(n, count)
     k_ms = kernel_ms / max(kernel_launches, 1)
     achieved = FLOP_PER_INTERACTION * pairs_per_launch / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_TFLOPS, "traffic": FORCE_KERNEL_DRAM_TRAFFIC_BYTES,
-                "kernel": "force_kernel<4,1024,4,false,2>", "kernel_ms": k_ms,
+                "kernel": "force_kernel<%d,%d,4,false,2>" % (geo["targets_per_thread"],
+                                                             {3: 1024, 2: 512, 1: 256}[geo["targets_per_thread"]]),
+                "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / ms_step,
                 "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); "
                               "no FP32 figure in MEASURED_PEAKS.json",

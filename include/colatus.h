@@ -179,7 +179,7 @@ int64_t  colatus_launch_count(void);
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 
 /* Tuning overrides for measurements (0 restores the automatic choice):
- *   "targets_per_thread" in {0,1,2,4};  "source_splits" in [0,16]. */
+ *   "targets_per_thread" in {0,1,2,3};  "source_splits" in [0,16]. */
 int colatus_set_option(const char *name, int64_t value);
 
 const char *colatus_last_error(void);

@@ -103,7 +103,7 @@ Workspace workspace_layout(int64_t n_max) {
 // Pick (I, TJ) and the source split so that CTAs ~ k * (SMs * CTAs/SM) with little padding
 // (DESIGN.md "Launch geometry").
 Geometry choose_geometry(int64_t n, int64_t t_count) {
-    static const int variants[3][2] = {{4, 1024}, {2, 512}, {1, 256}};
+    static const int variants[3][2] = {{3, 1024}, {2, 512}, {1, 256}};
     const int64_t slots = (int64_t)g.sm_count * g.ctas_per_sm;
     Geometry best;
     for (int v = 0; v < 3; ++v) {
@@ -159,8 +159,8 @@ cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const floa
                          int64_t t_count, float eps2, float scale, int final_out, float4 *out, int64_t out_stride,
                          cudaStream_t st) {
     switch (geo.I) {
-        case 4:
-            return launch_force_variant<4, 1024, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
+        case 3:
+            return launch_force_variant<3, 1024, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
                                                       final_out, out, out_stride, st);
         case 2:
             return launch_force_variant<2, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
@@ -582,7 +582,7 @@ int colatus_set_option(const char *name, int64_t value) {
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!name) return fail(COLATUS_INVALID_ARG, "name is null");
     if (!strcmp(name, "targets_per_thread")) {
-        if (value != 0 && value != 1 && value != 2 && value != 4) return fail(COLATUS_INVALID_ARG, "must be 0,1,2,4");
+        if (value < 0 || value > 3) return fail(COLATUS_INVALID_ARG, "must be 0,1,2,3");
         g.force_I = (int)value;
     } else if (!strcmp(name, "source_splits")) {
         if (value < 0 || value > MAX_SPLITS) return fail(COLATUS_INVALID_ARG, "must be in [0, %d]", MAX_SPLITS);
