@@ -239,8 +239,8 @@ def run_native(args):
     achieved = FLOP_PER_INTERACTION * pairs_per_launch / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_TFLOPS, "traffic": FORCE_KERNEL_DRAM_TRAFFIC_BYTES,
-                "kernel": "force_kernel<%d,%d,4,false,2>" % (geo["targets_per_thread"],
-                                                             {3: 1024, 2: 512, 1: 256}[geo["targets_per_thread"]]),
+                "kernel": "force_kernel<%d,%d,4,false,2>" % (geo["targets_per_thread"] // 2,
+                                                             {6: 512, 4: 512, 2: 256}[geo["targets_per_thread"]]),
                 "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / ms_step,
                 "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); "

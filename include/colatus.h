@@ -175,11 +175,11 @@ int64_t  colatus_launch_count(void);
 /* Geometry the force path picked for n bodies / target_count targets on this device:
  * out[0] = targets per CTA, out[1] = target tiles, out[2] = source splits,
  * out[3] = sources per split (padded), out[4] = CTAs per SM, out[5] = SM count,
- * out[6] = kernel variant (targets per thread), out[7] = threads per CTA. */
+ * out[6] = kernel variant (targets per thread = 2 x target pairs), out[7] = threads per CTA. */
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 
 /* Tuning overrides for measurements (0 restores the automatic choice):
- *   "targets_per_thread" in {0,1,2,3};  "source_splits" in [0,16]. */
+ *   "targets_per_thread" in {0,2,4,6};  "source_splits" in [0,16]. */
 int colatus_set_option(const char *name, int64_t value);
 
 const char *colatus_last_error(void);

@@ -25,7 +25,7 @@ constexpr int DIAG_BLOCKS_MAX = 1024;
 constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
 
 struct Geometry {
-    int I = 0, TJ = 0;
+    int IP = 0, TJ = 0;   // target pairs per thread, sources per tile
     int64_t tiles_t = 0;
     int splits = 0, tiles_per_split = 0;
     int64_t n_pad = 0;   // sources covered = splits * tiles_per_split * TJ
@@ -103,13 +103,14 @@ Workspace workspace_layout(int64_t n_max) {
 // Pick (I, TJ) and the source split so that CTAs ~ k * (SMs * CTAs/SM) with little padding
 // (DESIGN.md "Launch geometry").
 Geometry choose_geometry(int64_t n, int64_t t_count) {
-    static const int variants[3][2] = {{3, 1024}, {2, 512}, {1, 256}};
+    static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 256}};   // (target pairs per thread, tile)
     const int64_t slots = (int64_t)g.sm_count * g.ctas_per_sm;
     Geometry best;
     for (int v = 0; v < 3; ++v) {
-        const int I = variants[v][0], TJ = variants[v][1];
-        if (g.force_I && g.force_I != I) continue;
-        const int64_t tiles_t = (t_count + (int64_t)FORCE_THREADS * I - 1) / ((int64_t)FORCE_THREADS * I);
+        const int IP = variants[v][0], TJ = variants[v][1];
+        if (g.force_I && g.force_I != 2 * IP) continue;
+        const int64_t per_cta = (int64_t)FORCE_THREADS * 2 * IP;
+        const int64_t tiles_t = (t_count + per_cta - 1) / per_cta;
         const int64_t src_tiles = (n + TJ - 1) / TJ;
         const int64_t smax = src_tiles < MAX_SPLITS ? src_tiles : MAX_SPLITS;
         if (!g.force_I && v < 2 && tiles_t * smax < slots) continue;   // too few CTAs: finer variant
@@ -123,7 +124,7 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
             eff *= (double)tps / ((double)tps + 0.125);   // per-CTA prologue/epilogue
             if (eff > best_eff * 1.002) {                 // prefer fewer splits on near ties
                 best_eff = eff;
-                best.I = I;
+                best.IP = IP;
                 best.TJ = TJ;
                 best.tiles_t = tiles_t;
                 best.splits = (int)s;
@@ -136,12 +137,12 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
     return best;
 }
 
-template <int I, int TJ, bool POT>
+template <int IP, int TJ, bool POT>
 cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
                                  int64_t t_count, float eps2, float scale, int final_out, float4 *out,
                                  int64_t out_stride, cudaStream_t st) {
-    auto kern = force_kernel<I, TJ, NSTAGES, POT, 2>;
-    const size_t smem = (size_t)NSTAGES * TJ * 16 + 2 * NSTAGES * sizeof(uint64_t);
+    auto kern = force_kernel<IP, TJ, NSTAGES, POT, 2>;
+    const size_t smem = force_smem_bytes<IP, TJ, NSTAGES, POT>();
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -158,9 +159,9 @@ template <bool POT>
 cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
                          int64_t t_count, float eps2, float scale, int final_out, float4 *out, int64_t out_stride,
                          cudaStream_t st) {
-    switch (geo.I) {
+    switch (geo.IP) {
         case 3:
-            return launch_force_variant<3, 1024, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
+            return launch_force_variant<3, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
                                                       final_out, out, out_stride, st);
         case 2:
             return launch_force_variant<2, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
@@ -171,7 +172,7 @@ cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const floa
     }
 }
 
-// repack + force (+ reduce): the whole of step a3.  No validation here.
+// stage + force (+ reduce): the whole of step a3.  No validation here.
 int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2, float4 *out,
                bool potential, cudaStream_t st) {
     const Workspace w = workspace_layout(n);
@@ -182,8 +183,7 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
     float4 *partials = reinterpret_cast<float4 *>(g.ws + w.partials);
 
-    const int64_t pairs = geo.n_pad / 2;
-    repack_sources_kernel<<<(unsigned)((pairs + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed);
+    stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed);
     CUDA_TRY(cudaGetLastError());
     g.launches++;
 
@@ -567,13 +567,13 @@ int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]) {
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!out || n < 1 || target_count < 1 || target_count > n) return fail(COLATUS_INVALID_ARG, "bad arguments");
     const Geometry geo = choose_geometry(n, target_count);
-    out[0] = (int64_t)FORCE_THREADS * geo.I;
+    out[0] = (int64_t)FORCE_THREADS * 2 * geo.IP;
     out[1] = geo.tiles_t;
     out[2] = geo.splits;
     out[3] = (int64_t)geo.tiles_per_split * geo.TJ;
     out[4] = g.ctas_per_sm;
     out[5] = g.sm_count;
-    out[6] = geo.I;
+    out[6] = 2 * geo.IP;
     out[7] = FORCE_THREADS;
     return COLATUS_OK;
 }
@@ -582,7 +582,7 @@ int colatus_set_option(const char *name, int64_t value) {
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!name) return fail(COLATUS_INVALID_ARG, "name is null");
     if (!strcmp(name, "targets_per_thread")) {
-        if (value < 0 || value > 3) return fail(COLATUS_INVALID_ARG, "must be 0,1,2,3");
+        if (value != 0 && value != 2 && value != 4 && value != 6) return fail(COLATUS_INVALID_ARG, "must be 0,2,4,6");
         g.force_I = (int)value;
     } else if (!strcmp(name, "source_splits")) {
         if (value < 0 || value > MAX_SPLITS) return fail(COLATUS_INVALID_ARG, "must be in [0, %d]", MAX_SPLITS);

@@ -3,13 +3,14 @@
 //   F_k = G * sum_{j != k} m_j (x_j - x_k) / (|x_j - x_k|^2 + eps^2)^{3/2}
 //
 // Design:
-//   * repack kernel  : float4 (x,y,z,m)[n] -> source PAIRS (x0,x1,y0,y1)(z0,z1,m0,m1), zero-mass
-//                      padding, so one 64-bit register holds the same coordinate of two sources;
-//   * force kernel   : targets in registers (I per thread), source tiles staged in shared memory
-//                      by 1-D bulk async copies (cp.async.bulk + mbarrier ring) and read as
+//   * staging kernel : float4 (x,y,z,m)[n] -> the same array padded with zero-mass bodies to whole tiles;
+//   * force kernel   : target PAIRS in registers (IP pairs = 2*IP targets per thread, one 64-bit
+//                      register = the same coordinate of two targets), source tiles staged in shared
+//                      memory by 1-D bulk async copies (cp.async.bulk + mbarrier ring) and read as
 //                      warp-broadcast LDS.128; arithmetic in packed FP32 (fma/add/mul.rn.f32x2 ->
-//                      FFMA2/FADD2/FMUL2: two interactions per issue slot), rsqrt.approx on the
-//                      MUFU pipe; accumulators flushed once per tile (blocked summation);
+//                      FFMA2/FADD2/FMUL2: two interactions per issue slot) with the source scalars as
+//                      broadcast operands, rsqrt.approx on the MUFU pipe; accumulators flushed once
+//                      per tile (blocked summation);
 //   * the (target-tile x source-split) grid is sized to the machine, each split writes a
 //     partial sum, and a fixed-order reduce kernel adds the partials and applies G.
 // The self term needs no branch: d = 0 gives w*d = 0 exactly because eps^2 > 0 (reading G4).
@@ -92,46 +93,53 @@ __device__ __forceinline__ void bulk_copy_g2s(void *dst_smem, const void *src_gm
                  : "memory");
 }
 
-// ---- repack: AoS float4 -> source pairs -----------------------------------------------------------
-// packed[2p]   = (x_{2p}, x_{2p+1}, y_{2p}, y_{2p+1})
-// packed[2p+1] = (z_{2p}, z_{2p+1}, m_{2p}, m_{2p+1})        for p in [0, n_pad/2)
-// Sources j >= n are padding: position 0, mass 0 (contribute exactly 0 to F and to phi).
-__global__ void __launch_bounds__(256) repack_sources_kernel(const float4 *__restrict__ pos_mass, int64_t n,
-                                                             int64_t n_pad, float4 *__restrict__ packed) {
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (2 * p >= n_pad) return;
-    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    const float4 b0 = (2 * p < n) ? __ldg(pos_mass + 2 * p) : zero;
-    const float4 b1 = (2 * p + 1 < n) ? __ldg(pos_mass + 2 * p + 1) : zero;
-    packed[2 * p] = make_float4(b0.x, b1.x, b0.y, b1.y);
-    packed[2 * p + 1] = make_float4(b0.z, b1.z, b0.w, b1.w);
+// ---- staging: zero-mass padding of the source array -------------------------------------------------
+// staged[j] = pos_mass[j] for j < n, (0,0,0,0) for n <= j < n_pad.  Padding sources have mass 0 at a
+// finite position: they contribute exactly 0 to F and to phi (reading G4).  Every tile the force
+// kernel copies is then full, so its bulk copies and its inner loop need no tail handling.
+__global__ void __launch_bounds__(256) stage_sources_kernel(const float4 *__restrict__ pos_mass, int64_t n,
+                                                            int64_t n_pad, float4 *__restrict__ staged) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_pad) return;
+    staged[j] = (j < n) ? __ldg(pos_mass + j) : make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // ---- the force kernel -----------------------------------------------------------------------------
-// Template: I = targets per thread, TJ = sources per shared-memory tile (= accumulation block),
-// NST = ring stages, POT = also accumulate sum_j m_j / sqrt(r^2+eps^2), MINB = CTAs per SM.
-// grid = (target tiles, source splits); block = THREADS.
-//   targets of CTA bx : t0 + bx*THREADS*I + i*THREADS + tid,  i < I   (coalesced loads/stores)
-//   sources of split by: packed pairs [by*tiles_per_split*TJ/2, ...), tiles_per_split tiles
+// Template: IP = target PAIRS per thread (2*IP targets), TJ = sources per shared-memory tile
+// (= first-level accumulation block), NST = ring stages, POT = also accumulate
+// sum_j m_j / sqrt(r^2+eps^2), MINB = CTAs per SM.   grid = (target tiles, source splits).
+//   targets of CTA bx : t0 + bx*THREADS*2*IP + i*2*THREADS + 2*tid + {0,1},  i < IP
+//   sources of split by: staged[by*tiles_per_split*TJ ...), tiles_per_split tiles of TJ bodies
+// Packing is along TARGETS: one 64-bit register holds the same coordinate of two targets, and the
+// four floats of a source (one warp-broadcast LDS.128) enter as scalar-broadcast operands
+// (FADD2 R, R.F32x2, R.F32), so one shared-memory load serves 2*IP targets and the two halves of an
+// accumulator belong to different targets (no cross-half add at the flush).
+// Second-level accumulators live in shared memory (one packed add per tile per component).
 // Output: out[(by * out_stride) + target] = (sum_x, sum_y, sum_z, sum_pot) * scale  (scale = G when
 // there is a single split and the result is final, else 1 and the reduce kernel applies G).
 constexpr int FORCE_THREADS = 256;
 
-template <int I, int TJ, int NST, bool POT, int MINB>
+template <int IP, int TJ, int NST, bool POT>
+constexpr size_t force_smem_bytes() {
+    return (size_t)NST * TJ * 16 + 2 * NST * sizeof(uint64_t) + (size_t)IP * (POT ? 4 : 3) * FORCE_THREADS * 8;
+}
+
+template <int IP, int TJ, int NST, bool POT, int MINB>
 __global__ void __launch_bounds__(FORCE_THREADS, MINB)
-force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ packed, int64_t t_begin,
+force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ staged, int64_t t_begin,
              int64_t t_count, int tiles_per_split, float eps2, float scale, int final_out,
              float4 *__restrict__ out, int64_t out_stride) {
     constexpr int TILE_BYTES = TJ * 16;
+    constexpr int NC = POT ? 4 : 3;                                                  // components per target
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    ulonglong2 *tile = reinterpret_cast<ulonglong2 *>(smem_raw);                    // [NST][TJ] ulonglong2 (= TJ/2 pairs x 2)
     uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem_raw + NST * TILE_BYTES);  // [NST]
     uint64_t *empty_bar = full_bar + NST;                                            // [NST]
+    u64 *acc2 = reinterpret_cast<u64 *>(smem_raw + NST * TILE_BYTES + 2 * NST * 8);  // [IP*NC][THREADS]
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const unsigned char *src =
-        reinterpret_cast<const unsigned char *>(packed) + (size_t)blockIdx.y * tiles_per_split * TILE_BYTES;
+        reinterpret_cast<const unsigned char *>(staged) + (size_t)blockIdx.y * tiles_per_split * TILE_BYTES;
 
     if (tid == 0) {
 #pragma unroll
@@ -151,45 +159,45 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ pac
             }
     }
 
-    // targets: negated and duplicated so that d = x_j + (-x_k) is one packed add
-    u64 nx[I], ny[I], nz[I];
-    const int64_t tbase = (int64_t)blockIdx.x * (FORCE_THREADS * I) + tid;
-    float self_m[I];
+    // target pairs, negated so that d = x_j + (-x_k) is one packed add with a broadcast source scalar
+    u64 nx[IP], ny[IP], nz[IP];
+    const int64_t tbase = (int64_t)blockIdx.x * (FORCE_THREADS * 2 * IP) + 2 * tid;
+    float self_m[IP][2];
 #pragma unroll
-    for (int i = 0; i < I; ++i) {
-        const int64_t t = tbase + (int64_t)i * FORCE_THREADS;
-        float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (t < t_count) b = __ldg(pos_mass + t_begin + t);
-        nx[i] = pack2(-b.x, -b.x);
-        ny[i] = pack2(-b.y, -b.y);
-        nz[i] = pack2(-b.z, -b.z);
-        self_m[i] = b.w;
+    for (int i = 0; i < IP; ++i) {
+        const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
+        float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+        if (t < t_count) b0 = __ldg(pos_mass + t_begin + t);
+        if (t + 1 < t_count) b1 = __ldg(pos_mass + t_begin + t + 1);
+        nx[i] = pack2(-b0.x, -b1.x);
+        ny[i] = pack2(-b0.y, -b1.y);
+        nz[i] = pack2(-b0.z, -b1.z);
+        self_m[i][0] = b0.w;
+        self_m[i][1] = b1.w;
     }
     const u64 eps2_2 = pack2(eps2, eps2);
-
-    float sx[I], sy[I], sz[I], sp[I];   // second-level accumulators (one add per tile)
 #pragma unroll
-    for (int i = 0; i < I; ++i) sx[i] = sy[i] = sz[i] = sp[i] = 0.f;
+    for (int c = 0; c < IP * NC; ++c) acc2[c * FORCE_THREADS + tid] = 0ull;   // private to this thread
 
     for (int t = 0; t < tiles_per_split; ++t) {
         const int stage = t % NST;
         const uint32_t parity = (t / NST) & 1;
         mbar_wait(&full_bar[stage], parity);
-        const ulonglong2 *tp = tile + (size_t)stage * TJ;
+        const float4 *tp = reinterpret_cast<const float4 *>(smem_raw + (size_t)stage * TILE_BYTES);
 
-        u64 ax[I], ay[I], az[I], ap[I];
+        u64 ax[IP], ay[IP], az[IP], ap[IP];
 #pragma unroll
-        for (int i = 0; i < I; ++i) ax[i] = ay[i] = az[i] = ap[i] = 0ull;   // (+0.f, +0.f)
+        for (int i = 0; i < IP; ++i) ax[i] = ay[i] = az[i] = ap[i] = 0ull;   // (+0.f, +0.f)
 
 #pragma unroll 4
-        for (int p = 0; p < TJ / 2; ++p) {
-            const ulonglong2 A = tp[2 * p];       // (x0,x1) (y0,y1)
-            const ulonglong2 B = tp[2 * p + 1];   // (z0,z1) (m0,m1)
+        for (int j = 0; j < TJ; ++j) {
+            const float4 S = tp[j];                   // (x_j, y_j, z_j, m_j): same address in every lane
+            const u64 X = pack2(S.x, S.x), Y = pack2(S.y, S.y), Z = pack2(S.z, S.z), M = pack2(S.w, S.w);
 #pragma unroll
-            for (int i = 0; i < I; ++i) {
-                const u64 dx = add2(A.x, nx[i]);
-                const u64 dy = add2(A.y, ny[i]);
-                const u64 dz = add2(B.x, nz[i]);
+            for (int i = 0; i < IP; ++i) {
+                const u64 dx = add2(nx[i], X);
+                const u64 dy = add2(ny[i], Y);
+                const u64 dz = add2(nz[i], Z);
                 u64 r2 = fma2(dx, dx, eps2_2);
                 r2 = fma2(dy, dy, r2);
                 r2 = fma2(dz, dz, r2);
@@ -197,7 +205,7 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ pac
                 unpack2(r2, r2a, r2b);
                 const u64 rinv = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));
                 const u64 rinv2 = mul2(rinv, rinv);
-                const u64 mr = mul2(B.y, rinv);
+                const u64 mr = mul2(rinv, M);
                 const u64 w = mul2(mr, rinv2);
                 ax[i] = fma2(w, dx, ax[i]);
                 ay[i] = fma2(w, dy, ay[i]);
@@ -214,35 +222,39 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ pac
             bulk_copy_g2s(smem_raw + stage * TILE_BYTES, src + (size_t)(t + NST) * TILE_BYTES, TILE_BYTES,
                           &full_bar[stage]);
         }
-        // flush: even-source + odd-source halves, then into the per-split sum
+        // flush the tile's sums into the per-split sums (blocked summation)
 #pragma unroll
-        for (int i = 0; i < I; ++i) {
-            float lo, hi;
-            unpack2(ax[i], lo, hi);
-            sx[i] += lo + hi;
-            unpack2(ay[i], lo, hi);
-            sy[i] += lo + hi;
-            unpack2(az[i], lo, hi);
-            sz[i] += lo + hi;
-            if (POT) {
-                unpack2(ap[i], lo, hi);
-                sp[i] += lo + hi;
-            }
+        for (int i = 0; i < IP; ++i) {
+            u64 *a2 = acc2 + (size_t)(i * NC) * FORCE_THREADS + tid;
+            a2[0] = add2(a2[0], ax[i]);
+            a2[FORCE_THREADS] = add2(a2[FORCE_THREADS], ay[i]);
+            a2[2 * FORCE_THREADS] = add2(a2[2 * FORCE_THREADS], az[i]);
+            if (POT) a2[3 * FORCE_THREADS] = add2(a2[3 * FORCE_THREADS], ap[i]);
         }
     }
 
     float4 *o = out + (size_t)blockIdx.y * out_stride;
+    const float rinv_eps = rsqrt_approx(eps2);
 #pragma unroll
-    for (int i = 0; i < I; ++i) {
-        const int64_t t = tbase + (int64_t)i * FORCE_THREADS;
-        if (t < t_count) {
-            float pot = 0.f;
-            if (POT) {
-                pot = sp[i];
-                // the j = k term m_k / eps was included by the branch-free loop: remove it once, when final
-                if (final_out) pot = -(pot - self_m[i] * rsqrt_approx(eps2));
+    for (int i = 0; i < IP; ++i) {
+        const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
+        const u64 *a2 = acc2 + (size_t)(i * NC) * FORCE_THREADS + tid;
+        float fx[2], fy[2], fz[2], fp[2] = {0.f, 0.f};
+        unpack2(a2[0], fx[0], fx[1]);
+        unpack2(a2[FORCE_THREADS], fy[0], fy[1]);
+        unpack2(a2[2 * FORCE_THREADS], fz[0], fz[1]);
+        if (POT) unpack2(a2[3 * FORCE_THREADS], fp[0], fp[1]);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (t + h < t_count) {
+                float pot = 0.f;
+                if (POT) {
+                    pot = fp[h];
+                    // the j = k term m_k / eps was included by the branch-free loop: remove it once, when final
+                    if (final_out) pot = -(pot - self_m[i][h] * rinv_eps);
+                }
+                o[t + h] = make_float4(fx[h] * scale, fy[h] * scale, fz[h] * scale, pot * scale);
             }
-            o[t] = make_float4(sx[i] * scale, sy[i] * scale, sz[i] * scale, pot * scale);
         }
     }
 }
