@@ -66,6 +66,9 @@ typedef struct colatus_config {
     unsigned flags;             /* COLATUS_FLAG_* */
 } colatus_config;
 
+/* Cosmological model of eq. (2): H0 and the four density parameters today. */
+typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosmo;
+
 /* Bytes of device workspace needed for problems up to n_max bodies: the repacked
  * source array, source-split partial sums, reduction scratch, and staging for the
  * host-buffer entry point.  Pure host arithmetic; 0 if n_max < 1. */
@@ -126,6 +129,33 @@ int colatus_step_coefficients(double tau, double a, double H, double out[4]);
  * Asynchronous. */
 int colatus_step_coeffs(double d1, double cv, double ck, double d2);
 
+/* ---- eq. (9): symplectic drift-kick-drift (reading G11) ---------------
+ * The resident "velocity" array then holds w = p/m = a^2 v (canonical momentum per unit mass).
+ *   D(tau/2): x += w * int_{t}^{t+tau/2} dt/a^2;   K(tau): w += F(x) * int_{t}^{t+tau} dt/a;
+ *   D(tau/2): x += w * int_{t+tau/2}^{t+tau} dt/a^2
+ * with F = eq. (1) (the comoving potential of eq. (1) plays the role of phi' in eq. (8): d(a^2 v)/dt = F/a).
+ * colatus_symplectic_coefficients integrates eq. (2) from a(t) = a0 in double on the host and returns
+ * out = { d1, cv = 1, ck, d2, a(t+tau) }; host only.  colatus_step_symplectic enqueues the step with those
+ * coefficients (tracer tag = a(t+tau) as float) and returns a(t+tau) in *a_end (may be NULL).
+ * Requires c != NULL, a0 > 0, finite tau.  Asynchronous. */
+int colatus_symplectic_coefficients(const struct colatus_cosmo *c, double a0, double tau, double out[5]);
+int colatus_step_symplectic(const struct colatus_cosmo *c, double a0, double tau, double *a_end);
+
+/* ---- eq. (10): deformation-potential source (reading G21) -------------
+ * A fixed point source at x_psi of strength S = C*psi that "acts like a mass particle located in a fixed
+ * position": every force this library returns or uses gains
+ *   F_k += S (x_psi - x_k) / (|x_k - x_psi|^2 + eps^2)^{3/2}
+ * (attractive for S > 0; S is NOT multiplied by G, as in eq. (10)).  S = 0 disables (default).
+ * The term is not part of acc.w / W.  Applies to colatus_forces*, colatus_step* alike.  Host call. */
+int colatus_set_deformation(const double x_psi[3], double strength);
+
+/* Mean-density background term (reading G22; the paper states periodic/homogeneous
+ * boundaries, but prints no algorithm): every force gains
+ *   F_k += (4 pi / 3) G rho_bar (x_k - centre)
+ * which cancels the net pull of a homogeneous sphere of comoving density rho_bar about `centre`, so
+ * that an unperturbed box no longer contracts as a whole (G7).  rho_bar = 0 disables (default). */
+int colatus_set_background(const double centre[3], double rho_bar);
+
 /* Restrict the resident state to targets [target_begin, target_begin+target_count): only
  * those bodies are drifted, kicked and receive forces; all n bodies stay sources.  Used by
  * the target-sharded multi-GPU driver, which all-gathers positions between steps.
@@ -185,7 +215,6 @@ int colatus_set_option(const char *name, int64_t value);
 const char *colatus_last_error(void);
 
 /* ---- host-only cosmology, FP64 (eq. (2)) ---------------------------------- */
-typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosmo;
 
 /* H(a) = H0 sqrt(Om_R a^-4 + Om_M a^-3 + Om_K a^-2 + Om_L).  NaN if a <= 0. */
 double colatus_hubble(const colatus_cosmo *c, double a);

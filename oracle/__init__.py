@@ -48,6 +48,13 @@ def _load():
         lib.oracle_step_coeffs.argtypes = [c_void_p, c_void_p, c_void_p, c_int64, c_double, c_double,
                                            c_double, c_double, c_double, c_double, c_void_p]
         lib.oracle_step_coeffs.restype = None
+        lib.oracle_add_external.argtypes = [c_void_p, c_void_p, c_int64, c_double, c_double, c_void_p,
+                                            c_double, c_double, c_void_p, c_void_p]
+        lib.oracle_add_external.restype = None
+        lib.oracle_step_coeffs_ext.argtypes = [c_void_p, c_void_p, c_void_p, c_int64, c_double, c_double,
+                                               c_double, c_double, c_double, c_double,
+                                               c_double, c_void_p, c_double, c_void_p, c_void_p]
+        lib.oracle_step_coeffs_ext.restype = None
         lib.oracle_hubble.argtypes = [c_double] * 6
         lib.oracle_hubble.restype = c_double
         lib.oracle_a_advance.argtypes = [c_double] * 7 + [c_int]
@@ -100,6 +107,22 @@ def forces(pos_mass, eps2, G, targets=None, potential=False):
                      eps2, G, targets, potential)
 
 
+def add_external(x, acc, eps2, G, targets=None, deformation=None, background=None):
+    """Adds eq. (10) (deformation = (x_psi[3], S)) and / or the mean-density background term
+    (background = (centre[3], rho_bar)) to acc [k,3] for the targets (in place; returns acc)."""
+    x = _c64(x)
+    xpsi, S = (np.zeros(3), 0.0) if deformation is None else (_c64(deformation[0]), float(deformation[1]))
+    cen, rho = (np.zeros(3), 0.0) if background is None else (_c64(background[0]), float(background[1]))
+    if targets is None:
+        tptr, k = None, acc.shape[0]
+    else:
+        targets = np.ascontiguousarray(targets, dtype=np.int64)
+        tptr, k = _p(targets), targets.shape[0]
+    assert acc.dtype == np.float64 and acc.flags.c_contiguous and acc.shape == (k, 3)
+    _load().oracle_add_external(_p(x), tptr, k, float(eps2), S, _p(xpsi), float(G), rho, _p(cen), _p(acc))
+    return acc
+
+
 class State:
     """Double-precision simulation state started from the float32 input arrays."""
 
@@ -112,13 +135,37 @@ class State:
         self.eps2 = float(eps2)
         self.G = float(G)
         self._work = np.empty_like(self.x)
+        self.deformation = None      # (x_psi[3], S) of eq. (10), or None
+        self.background = None       # (centre[3], rho_bar), or None
 
     def step(self, tau, a, H):
         """Eqs. (3)-(5), PAPER.md:38-44."""
+        if self.deformation is not None or self.background is not None:
+            return self.step_coeffs(0.5 * tau, (1.0 - H * tau) / (1.0 + H * tau),
+                                    tau / (a ** 3 * (1.0 + H * tau)), 0.5 * tau)
         _load().oracle_step(_p(self.x), _p(self.v), _p(self.m), self.n, self.eps2, self.G,
                             float(tau), float(a), float(H), _p(self._work))
 
+    def step_symplectic(self, cosmo, a0, tau, panels=64, substeps=64):
+        """Eq. (9), PAPER.md:64 (reading G11): D(tau/2) K(tau) D(tau/2) in the variable w = a^2 v
+        (held in self.v).  Returns a(t + tau)."""
+        d1 = int_dt_over_a_pow(cosmo, a0, 0.5 * tau, 2.0, panels)
+        a_mid = a_advance(cosmo, a0, 0.5 * tau, substeps)
+        d2 = int_dt_over_a_pow(cosmo, a_mid, 0.5 * tau, 2.0, panels)
+        ck = int_dt_over_a_pow(cosmo, a0, tau, 1.0, panels)
+        self.step_coeffs(d1, 1.0, ck, d2)
+        return a_advance(cosmo, a_mid, 0.5 * tau, substeps)
+
     def step_coeffs(self, d1, cv, ck, d2):
+        if self.deformation is not None or self.background is not None:
+            xpsi, S = (np.zeros(3), 0.0) if self.deformation is None else \
+                (_c64(self.deformation[0]), float(self.deformation[1]))
+            cen, rho = (np.zeros(3), 0.0) if self.background is None else \
+                (_c64(self.background[0]), float(self.background[1]))
+            _load().oracle_step_coeffs_ext(_p(self.x), _p(self.v), _p(self.m), self.n, self.eps2, self.G,
+                                           float(d1), float(cv), float(ck), float(d2),
+                                           S, _p(xpsi), rho, _p(cen), _p(self._work))
+            return
         _load().oracle_step_coeffs(_p(self.x), _p(self.v), _p(self.m), self.n, self.eps2, self.G,
                                    float(d1), float(cv), float(ck), float(d2), _p(self._work))
 

@@ -21,6 +21,14 @@
  *                      P7 closed-form a(t) for EdS, flat LCDM, radiation,
  *                      matter+radiation, Milne, open matter+curvature, de Sitter
  *   oracle_diagnostics P9 momentum law, P11 Layzer-Irvine, static energy
+ *   oracle_step_coeffs / oracle_int_dt_over_a_pow (symplectic step of eq. 9)
+ *                      P12 EdS closed-form kick/drift integrals, exact sum m w
+ *                      conservation, force-free closed form, agreement with
+ *                      eqs. (3)-(5) as tau -> 0 at second order
+ *   oracle_add_external P13 extra-body equivalence + two-body closed form (eq. 10),
+ *                      linear closed form + homogeneous-sphere cancellation
+ *   oracle_splat       P14 brute-force counts, total = in-window particles
+ *   oracle_trace_spectrum P15 sinusoid closed form, Parseval, numpy FFT
  * Unpinned: nothing in this file.  (Physical realism of config 2 against the
  * paper's Fig. 1 statistics is "parity unpinned": it needs the paper's ICs.)
  *
@@ -127,6 +135,61 @@ void oracle_step_coeffs(double *x, double *v, const double *m, int64_t n, double
     int64_t i;
     for (i = 0; i < 3 * n; ++i) x[i] = x[i] + d1 * v[i];
     oracle_forces(x, m, n, eps2, G, NULL, n, work, NULL);
+    for (i = 0; i < 3 * n; ++i) v[i] = cv * v[i] + ck * work[i];
+    for (i = 0; i < 3 * n; ++i) x[i] = x[i] + d2 * v[i];
+}
+
+/*
+ * External terms added to the force of eq. (1) (NEXT rows f2 and f5 of SURVEY 8f):
+ *
+ *  (a) eq. (10): the deformation-potential source, a fixed point at
+ *      x_psi of strength S = C*psi which "acts like a mass particle located in a
+ *      fixed position"; attractive sign as in reading G1, S not
+ *      multiplied by G (reading G21):
+ *          F_k += S (x_psi - x_k) / (|x_k - x_psi|^2 + eps^2)^{3/2}
+ *  (b) mean-density background (reading G22; the paper asserts homogeneous /
+ *      periodic boundaries, without an algorithm):
+ *          F_k += (4 pi / 3) G rho_bar (x_k - centre)
+ *
+ * targets NULL = k = 0..n_targets-1.  acc [n_targets][3] is updated in place.
+ * Pins: (a) equals oracle_forces with one more body of mass S/G at x_psi, and the
+ * two-body closed form; (b) linear closed form, and cancellation of the pull of a
+ * homogeneous sphere (tests/test_oracle_pins.py).
+ */
+void oracle_add_external(const double *x, const int64_t *targets, int64_t n_targets, double eps2,
+                         double S, const double *x_psi, double G, double rho_bar, const double *centre,
+                         double *acc)
+{
+    const double pi = 3.14159265358979323846;
+    int64_t t;
+    for (t = 0; t < n_targets; ++t) {
+        const int64_t k = targets ? targets[t] : t;
+        if (S != 0.0) {
+            const double dx = x_psi[0] - x[3 * k], dy = x_psi[1] - x[3 * k + 1], dz = x_psi[2] - x[3 * k + 2];
+            const double s = dx * dx + dy * dy + dz * dz + eps2;
+            const double w = S / (s * sqrt(s));
+            acc[3 * t] += w * dx;
+            acc[3 * t + 1] += w * dy;
+            acc[3 * t + 2] += w * dz;
+        }
+        if (rho_bar != 0.0) {
+            const double B = (4.0 * pi / 3.0) * G * rho_bar;
+            acc[3 * t] += B * (x[3 * k] - centre[0]);
+            acc[3 * t + 1] += B * (x[3 * k + 1] - centre[1]);
+            acc[3 * t + 2] += B * (x[3 * k + 2] - centre[2]);
+        }
+    }
+}
+
+/* oracle_step_coeffs with the external terms above included in F. */
+void oracle_step_coeffs_ext(double *x, double *v, const double *m, int64_t n, double eps2, double G,
+                            double d1, double cv, double ck, double d2,
+                            double S, const double *x_psi, double rho_bar, const double *centre, double *work)
+{
+    int64_t i;
+    for (i = 0; i < 3 * n; ++i) x[i] = x[i] + d1 * v[i];
+    oracle_forces(x, m, n, eps2, G, NULL, n, work, NULL);
+    oracle_add_external(x, NULL, n, eps2, S, x_psi, G, rho_bar, centre, work);
     for (i = 0; i < 3 * n; ++i) v[i] = cv * v[i] + ck * work[i];
     for (i = 0; i < 3 * n; ++i) x[i] = x[i] + d2 * v[i];
 }

@@ -471,3 +471,139 @@ def test_layzer_irvine():
         res.append(abs(E[-1] - E[0] + integral))
         assert abs(E[-1] - E[0]) > 100 * res[-1]                            # non-vacuous: E changed a lot
     assert res[0] / res[1] == pytest.approx(4.0, rel=0.35)
+
+
+# ----------------------------------------------------------------------------- P12: symplectic step, eq. (9)
+def test_symplectic_force_free_closed_form():
+    """G = 0 in EdS: w = a^2 v is constant and x moves by w * int dt/a^2, which has a closed form
+    (a = (t/t1)^{2/3}: int dt/a^2 = -3 t1^{4/3} [t^{-1/3}])."""
+    H0 = EDS.H0
+    t1 = 2.0 / (3.0 * H0)
+    a0, tau, steps = 0.05, 2e-3, 7
+    t0 = t1 * a0 ** 1.5
+    x0 = RNG.random((4, 3))
+    w0 = RNG.normal(size=(4, 4))
+    w0[:, 3] = 0
+    st = oracle.State(_pm(x0, np.ones(4)), w0, 0.01, 0.0)
+    a = a0
+    for _ in range(steps):
+        a = st.step_symplectic(EDS, a, tau)
+    tf = t0 + steps * tau
+    assert a == pytest.approx((tf / t1) ** (2 / 3), rel=1e-9)
+    drift = -3.0 * t1 ** (4 / 3) * (tf ** (-1 / 3) - t0 ** (-1 / 3))
+    assert np.allclose(st.v, w0[:, :3], rtol=0, atol=0)                    # cv = 1 exactly
+    assert np.allclose(st.x, x0 + drift * w0[:, :3], rtol=1e-9)
+
+
+def test_symplectic_conserves_canonical_momentum_exactly():
+    """K adds ck * F with sum_k m_k F_k = 0 (P2) and cv = 1: sum m w is conserved to roundoff,
+    unlike eqs. (3)-(5) where it decays by the drag factor (P9)."""
+    n = 40
+    pm = _pm(RNG.random((n, 3)), RNG.random(n) / n)
+    w0 = np.concatenate([0.1 * RNG.normal(size=(n, 3)), np.zeros((n, 1))], axis=1)
+    st = oracle.State(pm, w0, 1e-3, 1.0)
+    P0 = (st.m[:, None] * st.v).sum(0)
+    a = 0.1
+    for _ in range(5):
+        a = st.step_symplectic(LCDM, a, 1e-4)
+    scale = (st.m[:, None] * np.abs(st.v)).sum()
+    assert np.abs((st.m[:, None] * st.v).sum(0) - P0).max() <= 1e-13 * scale
+    assert np.abs(st.v - w0[:, :3]).max() > 1e-3                            # non-vacuous: kicks happened
+
+
+def test_symplectic_static_limit_is_leapfrog():
+    """H0 -> 0 (a = 1): the integrals are tau/2, tau, tau/2 and eq. (9) is the plain D-K-D leapfrog."""
+    static = Cosmology(H0=1e-30, Om_L=1.0)
+    x, v, m, _ = _two_body_circular(0.04)
+    s1 = oracle.State(_pm(x, m), np.concatenate([v, np.zeros((2, 1))], 1), 0.04, 1.0)
+    s2 = oracle.State(_pm(x, m), np.concatenate([v, np.zeros((2, 1))], 1), 0.04, 1.0)
+    for _ in range(20):
+        s1.step_symplectic(static, 1.0, 0.01)
+        s2.step(0.01, 1.0, 0.0)
+    assert np.allclose(s1.x, s2.x, rtol=0, atol=1e-13) and np.allclose(s1.v, s2.v, rtol=0, atol=1e-13)
+
+
+def test_symplectic_and_eqs_3_5_converge_to_each_other():
+    """Both schemes integrate d(a^2 v)/dt = F/a: with v = w/a^2 their end states differ by O(tau^2)."""
+    n = 24
+    pm = _pm(RNG.random((n, 3)), np.full(n, 1.0 / n))
+    v0 = np.concatenate([0.3 * RNG.normal(size=(n, 3)), np.zeros((n, 1))], axis=1)
+    a0, T = 0.2, 0.02
+    diffs = []
+    for steps in (40, 80):
+        tau = T / steps
+        s1 = oracle.State(pm, v0, 0.05 ** 2, 1.0)
+        mids, ends = oracle.midstep_schedule(EDS, a0, tau, steps)
+        for a, H in mids:
+            s1.step(tau, a, H)
+        w0 = v0.copy()
+        w0[:, :3] *= a0 * a0
+        s2 = oracle.State(pm, w0, 0.05 ** 2, 1.0)
+        a = a0
+        for _ in range(steps):
+            a = s2.step_symplectic(EDS, a, tau)
+        assert a == pytest.approx(ends[-1], rel=1e-9)
+        diffs.append(np.abs(s1.x - s2.x).max() + np.abs(s1.v - s2.v / a ** 2).max())
+        assert np.abs(s1.x - pm[:, :3]).max() > 100 * diffs[-1]            # non-vacuous
+    assert diffs[0] / diffs[1] == pytest.approx(4.0, rel=0.25)
+
+
+# ----------------------------------------------------------------------------- P13: eq. (10) and background
+def test_deformation_source_is_a_fixed_extra_body():
+    """Eq. (10): the term 'acts like a mass particle located in a fixed position': it must
+    equal what eq. (1) gives when a body of mass S/G is appended at x_psi; and the two-body closed form."""
+    n, G, eps2, S = 17, 2.5, 0.03 ** 2, 0.7
+    x = RNG.random((n, 3))
+    m = RNG.random(n)
+    xpsi = np.array([0.3, -0.2, 1.1])
+    base = oracle.forces_xm(x, m, eps2, G)
+    got = oracle.add_external(x, base.copy(), eps2, G, deformation=(xpsi, S))
+    want = oracle.forces_xm(np.vstack([x, xpsi]), np.append(m, S / G), eps2, G)[:n]
+    assert np.allclose(got, want, rtol=1e-13, atol=1e-15)
+    d = xpsi - x[3]
+    r2 = d @ d
+    assert np.allclose(got[3] - base[3], S * d / (r2 + eps2) ** 1.5, rtol=1e-14)      # toward x_psi
+    sub = oracle.add_external(x, base[[5, 2]].copy(), eps2, G, targets=[5, 2], deformation=(xpsi, S))
+    assert np.allclose(sub, want[[5, 2]], rtol=1e-13)
+
+
+def test_background_term_closed_form_and_sphere_cancellation():
+    """F += (4 pi/3) G rho (x - c): linear closed form; and it cancels the pull of a homogeneous sphere
+    (shell theorem: -G M(<r)/r^2 = -(4 pi/3) G rho r) up to the discreteness of the lattice."""
+    G, rho = 1.7, 3.0
+    x = RNG.random((5, 3))
+    c = np.array([0.5, 0.4, 0.6])
+    got = oracle.add_external(x, np.zeros((5, 3)), 0.01, G, background=(c, rho))
+    assert np.allclose(got, (4 * math.pi / 3) * G * rho * (x - c), rtol=1e-15)
+    side = 28
+    g = (np.arange(side) + 0.5) / side - 0.5
+    X = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    X = X[(X ** 2).sum(1) <= 0.25]                                   # lattice points inside R = 0.5
+    m = np.full(len(X), 1.0 / side ** 3)                             # density 1
+    probes = np.array([[0.2, 0.1, -0.1], [-0.3, 0.05, 0.2], [0.0, 0.25, 0.0]])
+    pts = np.vstack([X, probes])
+    mm = np.append(m, np.zeros(3))                                   # massless probes
+    tg = np.arange(len(X), len(X) + 3)
+    grav = oracle.forces_xm(pts, mm, (0.5 / side) ** 2, G, tg)
+    tot = oracle.add_external(pts, grav.copy(), 0.0, G, targets=tg, background=(np.zeros(3), 1.0))
+    assert np.all(np.linalg.norm(tot, axis=1) <= 0.03 * np.linalg.norm(grav, axis=1))
+
+
+def test_step_with_external_terms_matches_composition():
+    """State.step with the external terms = drift, (eq. 1 + external), kick, drift written out here."""
+    n = 12
+    x0 = RNG.random((n, 3))
+    m = RNG.random(n) / n
+    v0 = 0.1 * RNG.normal(size=(n, 3))
+    st = oracle.State(_pm(x0, m), np.concatenate([v0, np.zeros((n, 1))], 1), 1e-3, 1.0)
+    st.deformation = (np.array([0.5, 0.5, 2.0]), 0.3)
+    st.background = (np.array([0.5, 0.5, 0.5]), 0.8)
+    tau, a, H = 1e-2, 0.5, 0.7
+    st.step(tau, a, H)
+    xh = x0 + 0.5 * tau * v0
+    F = oracle.forces_xm(xh, m, 1e-3, 1.0)
+    F = F + 0.3 * (st.deformation[0] - xh) / (((st.deformation[0] - xh) ** 2).sum(1, keepdims=True) + 1e-3) ** 1.5
+    F = F + (4 * math.pi / 3) * 0.8 * (xh - 0.5)
+    v1 = v0 * (1 - H * tau) / (1 + H * tau) + F * tau / (a ** 3 * (1 + H * tau))
+    assert np.allclose(st.v, v1, rtol=1e-12, atol=1e-15)
+    assert np.allclose(st.x, xh + 0.5 * tau * v1, rtol=1e-13)
