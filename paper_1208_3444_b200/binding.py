@@ -52,6 +52,10 @@ SIGNATURES = {
     "colatus_step": (c_int, [c_double, c_double, c_double]),
     "colatus_step_coefficients": (c_int, [c_double, c_double, c_double, POINTER(c_double)]),
     "colatus_step_coeffs": (c_int, [c_double, c_double, c_double, c_double]),
+    "colatus_symplectic_coefficients": (c_int, [POINTER(colatus_cosmo), c_double, c_double, POINTER(c_double)]),
+    "colatus_step_symplectic": (c_int, [POINTER(colatus_cosmo), c_double, c_double, POINTER(c_double)]),
+    "colatus_set_deformation": (c_int, [POINTER(c_double), c_double]),
+    "colatus_set_background": (c_int, [POINTER(c_double), c_double]),
     "colatus_set_target_range": (c_int, [c_int64, c_int64]),
     "colatus_drift": (c_int, [c_double]),
     "colatus_force_kick_drift": (c_int, [c_double, c_double, c_double]),
@@ -186,6 +190,32 @@ def colatus_step_coefficients(tau, a, H):
 
 def colatus_step_coeffs(d1, cv, ck, d2):
     _check(lib().colatus_step_coeffs(float(d1), float(cv), float(ck), float(d2)))
+
+
+def colatus_symplectic_coefficients(cosmo, a0, tau):
+    """Eq. (9): (d1, cv = 1, ck, d2, a_end), host only."""
+    out = (c_double * 5)()
+    _check(lib().colatus_symplectic_coefficients(ctypes.byref(_cosmo(cosmo)), float(a0), float(tau), out))
+    return tuple(out)
+
+
+def colatus_step_symplectic(cosmo, a0, tau):
+    """One symplectic drift-kick-drift step of eq. (9); returns a(t + tau)."""
+    a_end = c_double(0.0)
+    _check(lib().colatus_step_symplectic(ctypes.byref(_cosmo(cosmo)), float(a0), float(tau), ctypes.byref(a_end)))
+    return a_end.value
+
+
+def colatus_set_deformation(x_psi, strength):
+    """Eq. (10): fixed source of strength S = C*psi at x_psi; strength 0 disables."""
+    v = (c_double * 3)(*[float(c) for c in (x_psi if x_psi is not None else (0, 0, 0))])
+    _check(lib().colatus_set_deformation(v, float(strength)))
+
+
+def colatus_set_background(centre, rho_bar):
+    """Mean-density background term (reading G22); rho_bar 0 disables."""
+    v = (c_double * 3)(*[float(c) for c in (centre if centre is not None else (0, 0, 0))])
+    _check(lib().colatus_set_background(v, float(rho_bar)))
 
 
 def colatus_set_target_range(begin, count):

@@ -60,6 +60,8 @@ struct Context {
     int64_t launches = 0;
     // tuning overrides (0 = automatic)
     int force_I = 0, force_splits = 0;
+    // external terms: eq. (10) source and mean-density background (0 = off)
+    double def_S = 0.0, def_x[3] = {0, 0, 0}, bg_rho = 0.0, bg_c[3] = {0, 0, 0};
     char err[512] = "";
 };
 
@@ -222,6 +224,14 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         CUDA_TRY(cudaGetLastError());
         g.launches++;
     }
+    if (g.def_S != 0.0 || g.bg_rho != 0.0) {   // eq. (10) / background: O(n) epilogue on the finished forces
+        const double B = (4.0 * 3.14159265358979323846 / 3.0) * g.G * g.bg_rho;
+        external_field_kernel<<<(unsigned)((t_count + 255) / 256), 256, 0, st>>>(
+            pos_mass, t_begin, t_count, out, (float)g.def_S, (float)g.def_x[0], (float)g.def_x[1], (float)g.def_x[2],
+            eps2, (float)B, (float)g.bg_c[0], (float)g.bg_c[1], (float)g.bg_c[2]);
+        CUDA_TRY(cudaGetLastError());
+        g.launches++;
+    }
     return COLATUS_OK;
 }
 
@@ -313,6 +323,7 @@ int colatus_init(const colatus_config *cfg) {
     g.profile = false;
     g.ev_used = 0;
     g.force_I = g.force_splits = 0;
+    g.def_S = g.bg_rho = 0.0;
     g.initialised = true;
     g.err[0] = 0;
     return COLATUS_OK;
@@ -435,6 +446,61 @@ int colatus_step(double tau, double a, double H) {
     rc = enqueue_drift(c[0]);                                            // eq. (3)
     if (rc) return rc;
     return enqueue_force_kick_drift(c[1], c[2], c[3], (float)a);         // eqs. (1), (4), (5)
+}
+
+int colatus_symplectic_coefficients(const colatus_cosmo *c, double a0, double tau, double out[5]) {
+    if (!c || !out) return fail(COLATUS_INVALID_ARG, "null pointer");
+    if (!std::isfinite(a0) || !(a0 > 0.0) || !std::isfinite(tau)) return fail(COLATUS_INVALID_ARG, "a0 must be > 0, tau finite");
+    // eq. (9), PAPER.md:64 (reading G11): drift integrals of dt/a^2 over each half step, kick integral of dt/a
+    const double a_mid = colatus_a_advance(c, a0, 0.5 * tau);
+    out[0] = colatus_int_dt_over_a_pow(c, a0, 0.5 * tau, 2.0);
+    out[1] = 1.0;
+    out[2] = colatus_int_dt_over_a_pow(c, a0, tau, 1.0);
+    out[3] = colatus_int_dt_over_a_pow(c, a_mid, 0.5 * tau, 2.0);
+    out[4] = colatus_a_advance(c, a_mid, 0.5 * tau);
+    for (int i = 0; i < 5; ++i)
+        if (!std::isfinite(out[i])) return fail(COLATUS_INVALID_ARG, "scale-factor integration failed (a reached 0?)");
+    return COLATUS_OK;
+}
+
+int colatus_step_symplectic(const colatus_cosmo *c, double a0, double tau, double *a_end) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    double k[5];
+    int rc = colatus_symplectic_coefficients(c, a0, tau, k);
+    if (rc) return rc;
+    rc = enqueue_drift(k[0]);
+    if (rc) return rc;
+    rc = enqueue_force_kick_drift(k[1], k[2], k[3], (float)k[4]);
+    if (rc) return rc;
+    if (a_end) *a_end = k[4];
+    return COLATUS_OK;
+}
+
+int colatus_set_deformation(const double x_psi[3], double strength) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!std::isfinite(strength)) return fail(COLATUS_INVALID_ARG, "strength is not finite");
+    if (strength != 0.0) {
+        if (!x_psi) return fail(COLATUS_INVALID_ARG, "x_psi is null");
+        for (int i = 0; i < 3; ++i)
+            if (!std::isfinite(x_psi[i])) return fail(COLATUS_INVALID_ARG, "x_psi is not finite");
+        for (int i = 0; i < 3; ++i) g.def_x[i] = x_psi[i];
+    }
+    g.def_S = strength;
+    return COLATUS_OK;
+}
+
+int colatus_set_background(const double centre[3], double rho_bar) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!std::isfinite(rho_bar)) return fail(COLATUS_INVALID_ARG, "rho_bar is not finite");
+    if (rho_bar != 0.0) {
+        if (!centre) return fail(COLATUS_INVALID_ARG, "centre is null");
+        for (int i = 0; i < 3; ++i)
+            if (!std::isfinite(centre[i])) return fail(COLATUS_INVALID_ARG, "centre is not finite");
+        for (int i = 0; i < 3; ++i) g.bg_c[i] = centre[i];
+    }
+    g.bg_rho = rho_bar;
+    return COLATUS_OK;
 }
 
 int colatus_drift(double d) {

@@ -52,6 +52,33 @@ kick_drift_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, const
     }
 }
 
+// External terms added to the force of eq. (1) for the target range (acc indexed from 0):
+//   eq. (10), PAPER.md:93 (reading G21):  F_k += S (x_psi - x_k) / (|x_k - x_psi|^2 + eps^2)^{3/2}
+//   background (reading G22):             F_k += B (x_k - centre),  B = (4 pi / 3) G rho_bar (host, double)
+// O(n), IEEE division and square root (not on the hot path); acc.w is left alone.
+__global__ void __launch_bounds__(256)
+external_field_kernel(const float4 *__restrict__ pos_mass, int64_t begin, int64_t count, float4 *__restrict__ acc,
+                      float S, float px, float py, float pz, float eps2, float B, float cx, float cy, float cz) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const float4 p = pos_mass[begin + i];
+    float4 f = acc[i];
+    if (S != 0.f) {
+        const float dx = px - p.x, dy = py - p.y, dz = pz - p.z;
+        const float s = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+        const float w = S / (s * sqrtf(s));
+        f.x = fmaf(w, dx, f.x);
+        f.y = fmaf(w, dy, f.y);
+        f.z = fmaf(w, dz, f.z);
+    }
+    if (B != 0.f) {
+        f.x = fmaf(B, p.x - cx, f.x);
+        f.y = fmaf(B, p.y - cy, f.y);
+        f.z = fmaf(B, p.z - cz, f.z);
+    }
+    acc[i] = f;
+}
+
 // tracer slot map: slot[k] = t if idx[t] == k else -1
 __global__ void __launch_bounds__(256) trace_fill_kernel(int32_t *__restrict__ slot, int64_t n) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

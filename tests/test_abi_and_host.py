@@ -94,6 +94,29 @@ def test_eds():
         assert B.colatus_int_dt_over_a_pow(c, 0.1, 0.02, p) == pytest.approx(want, rel=1e-10)
 
 
+def test_symplectic_coefficients_eds_closed_form():
+    """Eq. (9) integrals in EdS, a = (t/t1)^{2/3}: int dt/a^p = t1^{2p/3} [t^q]/q, q = 1 - 2p/3."""
+    c = Cosmology(H0=2.894405, Om_M=1.0)
+    t1 = 2.0 / (3.0 * c.H0)
+    a0, tau = 0.1, 0.02
+    ta = t1 * a0 ** 1.5
+
+    def integral(p, t_from, t_to):
+        q = 1.0 - 2.0 * p / 3.0
+        return t1 ** (2 * p / 3) * (t_to ** q - t_from ** q) / q
+
+    d1, cv, ck, d2, a_end = B.colatus_symplectic_coefficients(c, a0, tau)
+    assert cv == 1.0
+    assert d1 == pytest.approx(integral(2.0, ta, ta + 0.5 * tau), rel=1e-10)
+    assert d2 == pytest.approx(integral(2.0, ta + 0.5 * tau, ta + tau), rel=1e-10)
+    assert ck == pytest.approx(integral(1.0, ta, ta + tau), rel=1e-10)
+    assert a_end == pytest.approx(((ta + tau) / t1) ** (2 / 3), rel=1e-11)
+    with pytest.raises(B.ColatusError):
+        B.colatus_symplectic_coefficients(c, 0.0, tau)
+    assert B.lib().colatus_set_deformation(None, 1.0) == B.NOT_INITIALISED
+    assert B.lib().colatus_set_background(None, 1.0) == B.NOT_INITIALISED
+
+
 def test_flat_lcdm():
     c = Cosmology(H0=70.0, Om_M=0.3, Om_L=0.7)
     f = lambda a: (2.0 / (3.0 * math.sqrt(0.7))) * math.asinh(math.sqrt(0.7 / 0.3) * a ** 1.5) / 70.0
