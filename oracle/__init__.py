@@ -66,6 +66,10 @@ def _load():
         lib.oracle_diagnostics.argtypes = [c_void_p, c_void_p, c_void_p, c_int64, c_double, c_double,
                                            c_double, c_int, c_void_p]
         lib.oracle_diagnostics.restype = None
+        lib.oracle_splat.argtypes = [c_void_p, c_int64, c_int, c_void_p, c_int, c_int, c_void_p]
+        lib.oracle_splat.restype = None
+        lib.oracle_trace_spectrum.argtypes = [c_void_p, c_int64, c_int64, c_void_p]
+        lib.oracle_trace_spectrum.restype = None
         del dp
         _lib = lib
     return _lib
@@ -121,6 +125,29 @@ def add_external(x, acc, eps2, G, targets=None, deformation=None, background=Non
     assert acc.dtype == np.float64 and acc.flags.c_contiguous and acc.shape == (k, 3)
     _load().oracle_add_external(_p(x), tptr, k, float(eps2), S, _p(xpsi), float(G), rho, _p(cen), _p(acc))
     return acc
+
+
+def splat(pos_mass, axis, window, width, height):
+    """Particle-count image of the positions (NEXT row f4; PAPER.md:115, Fig. 1 PAPER.md:83-85;
+    reading G23).  pos_mass: float32 [n,4]; window = (u0, u1, v0, v1, w0, w1).  uint32 [height, width]."""
+    pm = np.ascontiguousarray(pos_mass, dtype=np.float32)
+    assert pm.ndim == 2 and pm.shape[1] == 4
+    win = np.ascontiguousarray(window, dtype=np.float32)
+    assert win.shape == (6,)
+    img = np.empty((int(height), int(width)), dtype=np.uint32)
+    _load().oracle_splat(_p(pm), pm.shape[0], int(axis), _p(win), int(width), int(height), _p(img))
+    return img
+
+
+def trace_spectrum(series):
+    """Periodogram of the tracer velocity series (NEXT row f3; reading G24).
+    series: float32 [S, k, 4] rows of the tracer ring.  float64 [k, S//2 + 1]."""
+    sr = np.ascontiguousarray(series, dtype=np.float32)
+    assert sr.ndim == 3 and sr.shape[2] == 4
+    S, k = sr.shape[0], sr.shape[1]
+    out = np.empty((k, S // 2 + 1), dtype=np.float64)
+    _load().oracle_trace_spectrum(_p(sr), S, k, _p(out))
+    return out
 
 
 class State:

@@ -297,3 +297,93 @@ void oracle_diagnostics(const double *x, const double *v, const double *m, int64
         out[8] = NAN;
     }
 }
+
+/*
+ * Headless snapshot (NEXT row f4 of SURVEY 8f): the content of the paper's live
+ * display, "other library shows a particle motion in the box" (PAPER.md:115,
+ * App. A step 7) and of the Fig. 1 panels, as a particle-count
+ * image.  The paper gives no rendering algorithm; reading G23:
+ * orthographic projection along `axis`, one count per particle per pixel.
+ *
+ *   image axes (u, v) = the two other coordinates in cyclic order
+ *       axis 0: u = y, v = z;   axis 1: u = z, v = x;   axis 2: u = x, v = y
+ *   depth w = coordinate `axis`
+ *   window = (u0, u1, v0, v1, w0, w1): a particle is counted iff  w0 <= w < w1
+ *       and its pixel lies inside the image
+ *   pixel, decided in FP32 -- the precision of the device state -- with every
+ *   operation rounded once (this file is built with -ffp-contract=off):
+ *       su = (float)width / (u1 - u0),   tu = (u - u0) * su,   pu = floor(tu)
+ *       inside iff 0 <= tu < (float)width;       same for v with `height`
+ *   image[pv * width + pu] += 1        (row-major, uint32, zeroed first)
+ *
+ * pos_mass: float [n][4] (x, y, z, m) -- the same FP32 array the GPU gets.
+ * Pins (P14): brute force with exact rational arithmetic on dyadic inputs,
+ * total = number of in-window particles, marginals = numpy.histogram.
+ */
+void oracle_splat(const float *pos_mass, int64_t n, int axis, const float *window,
+                  int width, int height, uint32_t *image)
+{
+    const int iu = (axis + 1) % 3, iv = (axis + 2) % 3;
+    const float u0 = window[0], u1 = window[1], v0 = window[2], v1 = window[3];
+    const float w0 = window[4], w1 = window[5];
+    const float su = (float)width / (u1 - u0);
+    const float sv = (float)height / (v1 - v0);
+    for (int64_t p = 0; p < (int64_t)width * height; ++p) image[p] = 0u;
+    for (int64_t k = 0; k < n; ++k) {
+        const float u = pos_mass[4 * k + iu], v = pos_mass[4 * k + iv], w = pos_mass[4 * k + axis];
+        if (!(w >= w0 && w < w1)) continue;
+        const float du = u - u0;
+        const float tu = du * su;
+        const float dv = v - v0;
+        const float tv = dv * sv;
+        if (!(tu >= 0.0f && tu < (float)width)) continue;
+        if (!(tv >= 0.0f && tv < (float)height)) continue;
+        const int pu = (int)floorf(tu), pv = (int)floorf(tv);
+        image[(int64_t)pv * width + pu] += 1u;
+    }
+}
+
+/*
+ * Power spectrum of the velocity time series of each tracer particle (NEXT row
+ * f3 of SURVEY 8f): the paper's stated purpose for following single particles,
+ * "computation of the velocity of a single particle at every time-step ... and
+ * its energy power spectrum".  The paper gives no formula; reading
+ * G24: the periodogram of the recorded series, summed over the
+ * three velocity components,
+ *
+ *   P_t[f] = (1/S) sum_{c=x,y,z} | sum_{s=0}^{S-1} v_{t,c}[s] exp(-2 pi i f s / S) |^2,
+ *   f = 0 .. floor(S/2)                      (one-sided; real input)
+ *
+ * so that (Parseval)  sum over the full circle f = 0..S-1 of P_t[f] equals
+ * sum_s |v_t[s]|^2  = twice the tracer's kinetic energy per unit mass summed
+ * over the record.
+ *
+ * series: float [S][k][4] -- rows of the tracer ring, (vx, vy, vz, tag); the tag
+ * is ignored.  out: double [k][S/2 + 1].  Direct O(k S^2) evaluation of the
+ * definition; the phase is reduced exactly, (f s) mod S, before it is scaled.
+ * Pins (P15): a pure sinusoid (S A^2 / 4 in its own bin), a constant (S c^2 in
+ * bin 0), Parseval, and numpy.fft.rfft.
+ */
+void oracle_trace_spectrum(const float *series, int64_t S, int64_t k, double *out)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    const int64_t nf = S / 2 + 1;
+    int64_t t;
+#pragma omp parallel for schedule(static)
+    for (t = 0; t < k; ++t) {
+        for (int64_t f = 0; f < nf; ++f) {
+            double re[3] = {0, 0, 0}, im[3] = {0, 0, 0};
+            for (int64_t s = 0; s < S; ++s) {
+                const double ang = two_pi * (double)((f * s) % S) / (double)S;
+                const double c = cos(ang), sn = sin(ang);
+                for (int d = 0; d < 3; ++d) {
+                    const double val = (double)series[(s * k + t) * 4 + d];
+                    re[d] += val * c;
+                    im[d] -= val * sn;
+                }
+            }
+            out[t * nf + f] = (re[0] * re[0] + im[0] * im[0] + re[1] * re[1] + im[1] * im[1]
+                               + re[2] * re[2] + im[2] * im[2]) / (double)S;
+        }
+    }
+}

@@ -607,3 +607,138 @@ def test_step_with_external_terms_matches_composition():
     v1 = v0 * (1 - H * tau) / (1 + H * tau) + F * tau / (a ** 3 * (1 + H * tau))
     assert np.allclose(st.v, v1, rtol=1e-12, atol=1e-15)
     assert np.allclose(st.x, xh + 0.5 * tau * v1, rtol=1e-13)
+
+
+# ----------------------------------------------------------------------------- P14: headless snapshot (f4)
+def _splat_rational(pos, axis, window, width, height):
+    """Brute force in exact rational arithmetic: valid when every input is dyadic and the scale
+    width/(u1-u0) is a power of two, so that the FP32 pixel decision of reading G23 is exact."""
+    iu, iv = (axis + 1) % 3, (axis + 2) % 3
+    u0, u1, v0, v1 = [Fraction(float(c)) for c in window[:4]]
+    w0, w1 = float(window[4]), float(window[5])                     # may be -inf / +inf (no slab)
+    img = [[0] * width for _ in range(height)]
+    for p in pos:
+        u, v, w = Fraction(float(p[iu])), Fraction(float(p[iv])), Fraction(float(p[axis]))
+        if not (w0 <= w < w1):
+            continue
+        tu, tv = (u - u0) * width / (u1 - u0), (v - v0) * height / (v1 - v0)
+        if 0 <= tu < width and 0 <= tv < height:
+            img[math.floor(tv)][math.floor(tu)] += 1
+    return np.array(img, dtype=np.uint32)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_splat_brute_force_exact_on_dyadic_inputs(axis):
+    """Pixel = floor((u - u0) W / (u1 - u0)); image axes (u, v) cyclic after `axis`; slab on the depth."""
+    n = 3000
+    pos = (RNG.integers(-256, 1280, size=(n, 3)) / 1024.0).astype(np.float32)   # dyadic, some outside [0,1)
+    pm = np.concatenate([pos, np.ones((n, 1), np.float32)], 1)
+    for window, (W, H) in ((((0.0, 1.0, 0.0, 1.0, 0.25, 0.75)), (32, 16)),
+                           ((-0.25, 0.75, 0.5, 1.0, -np.inf, np.inf), (64, 8)),
+                           ((0.5, 0.625, 0.0, 0.25, 0.0, 1.0), (4, 4))):
+        got = oracle.splat(pm, axis, window, W, H)
+        want = _splat_rational(pos, axis, window, W, H)
+        assert got.dtype == np.uint32 and got.shape == (H, W)
+        assert np.array_equal(got, want)
+        assert want.sum() > 0
+
+
+def test_splat_total_and_marginals_match_numpy_histogram():
+    """Sum of the image = particles inside window and slab; its marginals = numpy.histogram of u and v
+    (inputs dyadic with a power-of-two bin width, so numpy's FP64 binning is exact as well)."""
+    n = 20000
+    pos = (RNG.integers(0, 4096, size=(n, 3)) / 4096.0).astype(np.float32)
+    pm = np.concatenate([pos, np.zeros((n, 1), np.float32)], 1)
+    img = oracle.splat(pm, 2, (0.0, 1.0, 0.0, 1.0, 0.125, 0.5), 64, 32)
+    sel = (pos[:, 2] >= 0.125) & (pos[:, 2] < 0.5)
+    assert img.sum() == sel.sum()
+    hu, _ = np.histogram(pos[sel, 0].astype(np.float64), bins=64, range=(0.0, 1.0))
+    hv, _ = np.histogram(pos[sel, 1].astype(np.float64), bins=32, range=(0.0, 1.0))
+    assert np.array_equal(img.sum(0), hu) and np.array_equal(img.sum(1), hv)
+    # the upper edges are exclusive: a particle exactly at u1 is not counted (numpy's last bin is closed)
+    edge = np.array([[1.0, 0.5, 0.25, 1.0], [0.5, 1.0, 0.25, 1.0], [0.5, 0.5, 0.5, 1.0], [0.0, 0.0, 0.125, 1.0]],
+                    dtype=np.float32)
+    e = oracle.splat(edge, 2, (0.0, 1.0, 0.0, 1.0, 0.125, 0.5), 4, 4)
+    assert e.sum() == 1 and e[0, 0] == 1
+
+
+def test_splat_pixel_decision_is_fp32():
+    """Reading G23: the pixel is decided in FP32, (u - u0) * (W / (u1 - u0)) with each op rounded once.
+    Independent restatement with numpy float32 scalars on non-dyadic inputs."""
+    n = 5000
+    pos = RNG.random((n, 3)).astype(np.float32)
+    pm = np.concatenate([pos, np.ones((n, 1), np.float32)], 1)
+    win = np.array([0.1, 0.9, 0.2, 0.7, 0.0, 1.0], dtype=np.float32)
+    W, H = 37, 23
+    su = np.float32(W) / (win[1] - win[0])
+    sv = np.float32(H) / (win[3] - win[2])
+    tu = (pos[:, 1] - win[0]) * su          # axis 0: u = y, v = z
+    tv = (pos[:, 2] - win[2]) * sv
+    assert tu.dtype == np.float32
+    ok = (tu >= 0) & (tu < W) & (tv >= 0) & (tv < H)
+    want = np.zeros((H, W), dtype=np.uint32)
+    np.add.at(want, (np.floor(tv[ok]).astype(int), np.floor(tu[ok]).astype(int)), 1)
+    assert np.array_equal(oracle.splat(pm, 0, win, W, H), want)
+
+
+# ----------------------------------------------------------------------------- P15: tracer power spectrum (f3)
+def _series(v):
+    """[S, k, 3] -> ring rows [S, k, 4] float32."""
+    S, k, _ = v.shape
+    out = np.zeros((S, k, 4), dtype=np.float32)
+    out[:, :, :3] = v
+    out[:, :, 3] = 7.0          # the tag column must be ignored
+    return out
+
+
+def test_spectrum_sinusoid_and_constant_closed_forms():
+    """v_x[s] = A cos(2 pi f0 s / S + phi): P[f0] = S A^2 / 4 (0 < f0 < S/2), 0 elsewhere;
+    a constant c in v_y: P[0] = S c^2; Nyquist (-1)^s B in v_z: P[S/2] = S B^2."""
+    S, f0, A, phi, c, B = 64, 5, 0.75, 0.3, 0.5, 0.25
+    s = np.arange(S)
+    v = np.zeros((S, 2, 3))
+    v[:, 0, 0] = A * np.cos(2 * np.pi * f0 * s / S + phi)
+    v[:, 1, 1] = c
+    v[:, 1, 2] = B * (-1.0) ** s
+    ser = _series(v)
+    P = oracle.trace_spectrum(ser)
+    assert P.shape == (2, S // 2 + 1)
+    x32 = ser[:, 0, 0].astype(np.float64)                           # the float32-rounded series
+    want0 = np.zeros(S // 2 + 1)
+    want0[f0] = S * A * A / 4
+    assert np.allclose(P[0], want0, atol=2e-6 * S * A * A)          # float32 rounding of the samples
+    want1 = np.zeros(S // 2 + 1)
+    want1[0], want1[S // 2] = S * c * c, S * B * B
+    assert np.allclose(P[1], want1, atol=1e-12)                     # 0.5, +-0.25 are exact in float32
+    assert abs(P[0].sum() * 2 - (x32 ** 2).sum()) < 1e-5            # only interior bins are occupied
+
+
+@pytest.mark.parametrize("S", [16, 45, 100])
+def test_spectrum_parseval_and_numpy_rfft(S):
+    """Full-circle sum of P = sum_s |v[s]|^2 (one-sided bins doubled except 0 and Nyquist), and
+    P = sum_c |rfft(v_c)|^2 / S (special case: the definition is a DFT)."""
+    k = 5
+    ser = _series(RNG.normal(size=(S, k, 3)))
+    P = oracle.trace_spectrum(ser)
+    v = ser[:, :, :3].astype(np.float64)
+    wgt = np.full(S // 2 + 1, 2.0)
+    wgt[0] = 1.0
+    if S % 2 == 0:
+        wgt[-1] = 1.0
+    assert np.allclose((P * wgt).sum(1), (v ** 2).sum((0, 2)), rtol=1e-12)
+    F = np.fft.rfft(v, axis=0)                                      # [S//2+1, k, 3]
+    assert np.allclose(P, (np.abs(F) ** 2).sum(2).T / S, rtol=1e-10, atol=1e-12)
+
+
+def test_spectrum_time_shift_invariance_and_component_sum():
+    """A cyclic shift of the record changes only phases; components add."""
+    S, k = 40, 3
+    v = RNG.normal(size=(S, k, 3))
+    P = oracle.trace_spectrum(_series(v))
+    assert np.allclose(oracle.trace_spectrum(_series(np.roll(v, 7, axis=0))), P, rtol=1e-9, atol=1e-12)
+    parts = 0
+    for c in range(3):
+        vc = np.zeros_like(v)
+        vc[:, :, c] = v[:, :, c]
+        parts = parts + oracle.trace_spectrum(_series(vc))
+    assert np.allclose(parts, P, rtol=1e-12, atol=1e-14)
