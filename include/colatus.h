@@ -12,6 +12,8 @@
  *   - eq. (2), PAPER.md:33 : Friedmann equation, host only, double precision.
  *   - per-step velocities of selected tracer particles.
  *   - momentum / energy reductions (p = m a^2 v, eq. (7)).
+ *   - a headless particle-count snapshot (Fig. 1) and the power spectrum of
+ *     the tracer velocity series.
  *
  * Conventions
  *   - "body array" = float4 per particle, 16-byte aligned: positions carry
@@ -179,6 +181,35 @@ int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_st
  * fails with COLATUS_INVALID_ARG if the ring no longer (or not yet) holds them.
  * Synchronises the stream. */
 int colatus_trace_read(float *host_out, int64_t first_step, int n_steps);
+
+/* ---- headless snapshot (NEXT row f4; App. A step 7, Fig. 1) ------
+ * Particle-count image of the positions: the content of the paper's live display and of its
+ * Fig. 1 panels, without a window (reading G23 -- the paper gives no rendering algorithm).
+ * Orthographic projection along `axis` (0, 1, 2); image axes (u, v) = the two other
+ * coordinates in cyclic order (axis 0: u=y, v=z; axis 1: u=z, v=x; axis 2: u=x, v=y); depth
+ * w = coordinate `axis`.  window = (u0, u1, v0, v1, w0, w1) (host floats).  A body is counted
+ * iff w0 <= w < w1 and 0 <= tu < width and 0 <= tv < height, where, in FP32 with each operation
+ * rounded once, tu = (u - u0) * (width / (u1 - u0)), tv likewise; its pixel is
+ * image_dev[floor(tv) * width + floor(tu)] (uint32, row-major [height][width], caller-owned
+ * device memory, zeroed by this call).  Masses are ignored.  Counts are exact integers,
+ * independent of execution order.
+ * pos_mass_dev: device float4[n], or NULL for the resident state (then n is ignored and the
+ * work goes to the resident stream).  Requirements: u1 > u0, v1 > v0, w1 > w0; u/v bounds
+ * finite (w0, w1 may be -inf / +inf: no slab); 1 <= width, height <= 32768.  Asynchronous. */
+int colatus_splat(const void *pos_mass_dev, int64_t n, int axis, const float window[6], int width,
+                  int height, uint32_t *image_dev, void *cuda_stream);
+
+/* ---- tracer velocity power spectrum (NEXT row f3) -------------------------------
+ * "computation of the velocity of a single particle at every time-step ... and its energy
+ * power spectrum": periodogram of the recorded series of every tracer (reading G24 -- the
+ * paper gives no formula), summed over the velocity components:
+ *   P_t[f] = (1/S) sum_c | sum_{s<S} v_{t,c}[first_step + s] exp(-2 pi i f s / S) |^2,
+ *   f = 0 .. S/2,  S = n_steps,
+ * so that the full-circle sum of P_t equals sum_s |v_t[s]|^2 (Parseval).
+ * spectrum_dev: device double[k][S/2 + 1], caller-owned.  Direct O(k S^2) evaluation in FP64
+ * from the FP32 ring samples.  The ring must still hold steps [first_step, first_step + S)
+ * (as for colatus_trace_read); 2 <= S <= 65536.  Asynchronous on the resident stream. */
+int colatus_trace_spectrum(int64_t first_step, int n_steps, double *spectrum_dev);
 
 /* ---- diagnostics (eq. (7)) ------------------------------
  * Sums over the resident target range (all n bodies unless colatus_set_target_range):

@@ -61,6 +61,8 @@ SIGNATURES = {
     "colatus_force_kick_drift": (c_int, [c_double, c_double, c_double]),
     "colatus_trace": (c_int, [c_void_p, c_int, c_void_p, c_int]),
     "colatus_trace_read": (c_int, [c_void_p, c_int64, c_int]),
+    "colatus_splat": (c_int, [c_void_p, c_int64, c_int, POINTER(c_float), c_int, c_int, c_void_p, c_void_p]),
+    "colatus_trace_spectrum": (c_int, [c_int64, c_int, c_void_p]),
     "colatus_diagnostics": (c_int, [c_double, c_int, POINTER(c_double)]),
     "colatus_download": (c_int, [c_void_p, c_void_p]),
     "colatus_profile": (c_int, [c_int]),
@@ -236,6 +238,18 @@ def colatus_trace(idx, k, ring, capacity_steps):
 
 def colatus_trace_read(host_out, first_step, n_steps):
     _check(lib().colatus_trace_read(_host_ptr(host_out), int(first_step), int(n_steps)))
+
+
+def colatus_splat(pos_mass, n, axis, window, width, height, image, stream=None):
+    """Particle-count image (Fig. 1); pos_mass None = resident state."""
+    win = (c_float * 6)(*[float(c) for c in window])
+    _check(lib().colatus_splat(None if pos_mass is None else _ptr(pos_mass), int(n), int(axis), win,
+                               int(width), int(height), _ptr(image), _stream(stream)))
+
+
+def colatus_trace_spectrum(first_step, n_steps, spectrum):
+    """Periodogram of the tracer velocity series (PAPER.md:23) into a device double [k, n_steps//2+1]."""
+    _check(lib().colatus_trace_spectrum(int(first_step), int(n_steps), _ptr(spectrum)))
 
 
 def colatus_diagnostics(a, with_potential=False):

@@ -14,6 +14,7 @@
 #include "../../include/colatus.h"
 #include "force_kernels.cuh"
 #include "integrate_kernels.cuh"
+#include "analysis_kernels.cuh"
 
 namespace {
 
@@ -554,6 +555,60 @@ int colatus_trace_read(float *host_out, int64_t first_step, int n_steps) {
         s += run;
     }
     CUDA_TRY(cudaStreamSynchronize(g.stream));
+    return COLATUS_OK;
+}
+
+int colatus_splat(const void *pos_mass_dev, int64_t n, int axis, const float window[6], int width, int height,
+                  uint32_t *image_dev, void *cuda_stream) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    const float4 *pm = static_cast<const float4 *>(pos_mass_dev);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (!pm) {
+        if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "pos_mass_dev is null and colatus_upload has not been called");
+        pm = g.pos;
+        n = g.n;
+        st = g.stream;
+    }
+    if (!window || !image_dev) return fail(COLATUS_INVALID_ARG, "null pointer");
+    if (n < 1 || n > 2147483647LL) return fail(COLATUS_INVALID_ARG, "n=%lld out of [1, 2^31-1]", (long long)n);
+    if (!aligned16(pm) || (reinterpret_cast<uintptr_t>(image_dev) & 3u))
+        return fail(COLATUS_INVALID_ARG, "pointer misaligned");
+    if (axis < 0 || axis > 2) return fail(COLATUS_INVALID_ARG, "axis must be 0, 1 or 2");
+    if (width < 1 || width > 32768 || height < 1 || height > 32768)
+        return fail(COLATUS_INVALID_ARG, "width and height must be in [1, 32768]");
+    const float u0 = window[0], u1 = window[1], v0 = window[2], v1 = window[3], w0 = window[4], w1 = window[5];
+    if (!std::isfinite(u0) || !std::isfinite(u1) || !std::isfinite(v0) || !std::isfinite(v1) || !(u1 > u0) ||
+        !(v1 > v0) || !(w1 > w0))
+        return fail(COLATUS_INVALID_ARG, "window needs finite u0 < u1, v0 < v1 and w0 < w1");
+    const float su = (float)width / (u1 - u0);            // one IEEE single division each (reading G23)
+    const float sv = (float)height / (v1 - v0);
+    if (!std::isfinite(su) || !std::isfinite(sv)) return fail(COLATUS_INVALID_ARG, "window too narrow");
+    CUDA_TRY(cudaMemsetAsync(image_dev, 0, (size_t)width * height * sizeof(uint32_t), st));
+    splat_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pm, n, axis, u0, su, v0, sv, w0, w1, width, height,
+                                                              image_dev);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
+int colatus_trace_spectrum(int64_t first_step, int n_steps, double *spectrum_dev) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded || g.trace_k == 0) return fail(COLATUS_NOT_UPLOADED, "no tracers configured");
+    if (!spectrum_dev || (reinterpret_cast<uintptr_t>(spectrum_dev) & 7u))
+        return fail(COLATUS_INVALID_ARG, "spectrum_dev null or misaligned");
+    if (n_steps < 2 || n_steps > 65536 || first_step < 0)
+        return fail(COLATUS_INVALID_ARG, "need first_step >= 0 and 2 <= n_steps <= 65536");
+    if (first_step + n_steps > g.step || first_step < g.step - g.trace_cap)
+        return fail(COLATUS_INVALID_ARG, "steps [%lld, +%d) not held by the ring (step=%lld, capacity=%d)",
+                    (long long)first_step, n_steps, (long long)g.step, g.trace_cap);
+    const int nf = n_steps / 2 + 1;
+    const int bx = g.trace_k >= 32 ? 32 : (g.trace_k >= 16 ? 16 : 8);   // tracers across lanes
+    const dim3 block(bx, 256 / bx);
+    const dim3 grid((g.trace_k + block.x - 1) / block.x, (nf + block.y - 1) / block.y);
+    trace_spectrum_kernel<<<grid, block, 0, g.stream>>>(g.ring, g.trace_k, g.trace_cap, first_step, n_steps,
+                                                        spectrum_dev);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
     return COLATUS_OK;
 }
 

@@ -99,3 +99,19 @@ class Session:
 
     def diagnostics(self, a=1.0, with_potential=False):
         return np.array(B.colatus_diagnostics(a, with_potential))
+
+    # ---- NEXT rows f4, f3: snapshot image and tracer spectrum ------------------------------------------
+    def splat(self, axis, window, width, height, pos_mass=None) -> np.ndarray:
+        """Particle-count image uint32 [height, width] of `pos_mass` (numpy / CUDA tensor) or, if None,
+        of the resident positions."""
+        img = torch.empty((height, width), dtype=torch.int32, device=self.device)
+        pm = None
+        if pos_mass is not None:
+            pm = pos_mass if isinstance(pos_mass, torch.Tensor) else self.to_device(pos_mass)
+        B.colatus_splat(pm, 0 if pm is None else pm.shape[0], axis, window, width, height, img)
+        return img.cpu().numpy().view(np.uint32)
+
+    def trace_spectrum(self, first_step: int, n_steps: int) -> np.ndarray:
+        out = torch.empty((self.trace_k, n_steps // 2 + 1), dtype=torch.float64, device=self.device)
+        B.colatus_trace_spectrum(first_step, n_steps, out)
+        return out.cpu().numpy()
