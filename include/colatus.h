@@ -131,6 +131,26 @@ int colatus_step_coefficients(double tau, double a, double H, double out[4]);
  * Asynchronous. */
 int colatus_step_coeffs(double d1, double cv, double ck, double d2);
 
+/* ---- native step loop ("optionally replayed from a CUDA graph") -----------------------
+ * n_steps steps of eqs. (3)-(5) in one call, with the scale-factor schedule of eq. (2) formed
+ * on the host in double exactly as a caller of colatus_step would: for each step
+ *   a_mid = a(t_n + tau/2), H_mid = H(a_mid)  (reading G3),  then a(t_n + tau);
+ * c == NULL means a static background (a = 1, H = 0; a_start ignored).  The per-step
+ * coefficients go to a device table (in the workspace, 1024 steps per upload) and a device
+ * counter selects the row, so every step launches the same kernels with the same arguments:
+ * with use_graph != 0 one captured CUDA graph of the step (drift, stage, force, reduce,
+ * kick-drift + tracer record) is replayed per step -- this is what makes the launch-bound
+ * small-N loops (configs 1-3) fast; with use_graph == 0 the same kernels are launched one by
+ * one (for comparison).  Results are bitwise identical to n_steps calls of colatus_step.
+ * The loop runs on a stream owned by the library, ordered after everything already enqueued
+ * on the resident stream and before everything enqueued on it later.  *a_end (may be NULL)
+ * receives a(t_0 + n_steps tau).  Nothing is enqueued if any step's coefficients are invalid
+ * (colatus_step's checks).  The graph is re-captured after colatus_upload, colatus_trace,
+ * colatus_set_target_range, colatus_set_deformation / _background or colatus_set_option.
+ * Asynchronous. */
+int colatus_run(const struct colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph,
+                double *a_end);
+
 /* ---- eq. (9): symplectic drift-kick-drift (reading G11) ---------------
  * The resident "velocity" array then holds w = p/m = a^2 v (canonical momentum per unit mass).
  *   D(tau/2): x += w * int_{t}^{t+tau/2} dt/a^2;   K(tau): w += F(x) * int_{t}^{t+tau} dt/a;

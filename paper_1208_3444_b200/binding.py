@@ -52,6 +52,7 @@ SIGNATURES = {
     "colatus_step": (c_int, [c_double, c_double, c_double]),
     "colatus_step_coefficients": (c_int, [c_double, c_double, c_double, POINTER(c_double)]),
     "colatus_step_coeffs": (c_int, [c_double, c_double, c_double, c_double]),
+    "colatus_run": (c_int, [POINTER(colatus_cosmo), c_double, c_double, c_int64, c_int, POINTER(c_double)]),
     "colatus_symplectic_coefficients": (c_int, [POINTER(colatus_cosmo), c_double, c_double, POINTER(c_double)]),
     "colatus_step_symplectic": (c_int, [POINTER(colatus_cosmo), c_double, c_double, POINTER(c_double)]),
     "colatus_set_deformation": (c_int, [POINTER(c_double), c_double]),
@@ -192,6 +193,14 @@ def colatus_step_coefficients(tau, a, H):
 
 def colatus_step_coeffs(d1, cv, ck, d2):
     _check(lib().colatus_step_coeffs(float(d1), float(cv), float(ck), float(d2)))
+
+
+def colatus_run(cosmo, a_start, tau, n_steps, use_graph=True):
+    """n_steps steps of eqs. (3)-(5) in one native call (CUDA-graph replay); cosmo None = static.  Returns a_end."""
+    a_end = c_double(0.0)
+    cp = None if cosmo is None else ctypes.byref(_cosmo(cosmo))
+    _check(lib().colatus_run(cp, float(a_start), float(tau), int(n_steps), int(bool(use_graph)), ctypes.byref(a_end)))
+    return a_end.value
 
 
 def colatus_symplectic_coefficients(cosmo, a0, tau):

@@ -24,6 +24,7 @@ constexpr int MAX_SPLITS = 16;        // source splits (partials kept in the wor
 constexpr int NSTAGES = 4;            // shared-memory ring depth
 constexpr int DIAG_BLOCKS_MAX = 1024;
 constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
+constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in colatus_run
 
 struct Geometry {
     int IP = 0, TJ = 0;   // target pairs per thread, sources per tile
@@ -34,7 +35,7 @@ struct Geometry {
 
 struct Workspace {     // byte offsets inside the caller's workspace
     size_t packed = 0, partials = 0, scratch_acc = 0, trace_slot = 0, diag = 0, stage_in = 0, stage_out = 0,
-           total = 0;
+           step_table = 0, step_ctr = 0, total = 0;
 };
 
 struct Context {
@@ -63,6 +64,12 @@ struct Context {
     int force_I = 0, force_splits = 0;
     // external terms: eq. (10) source and mean-density background (0 = off)
     double def_S = 0.0, def_x[3] = {0, 0, 0}, bg_rho = 0.0, bg_c[3] = {0, 0, 0};
+    // colatus_run: private capture stream, ordering events, cached one-step graph
+    cudaStream_t run_stream = nullptr;
+    cudaEvent_t run_ev_in = nullptr, run_ev_out = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    bool graph_valid = false;
     char err[512] = "";
 };
 
@@ -99,6 +106,8 @@ Workspace workspace_layout(int64_t n_max) {
     w.diag = off;        off += round_up((size_t)(DIAG_BLOCKS_MAX + 2) * DIAG_Q * 8, 256);
     w.stage_in = off;    off += round_up(n * 16, 256);
     w.stage_out = off;   off += round_up(n * 16, 256);
+    w.step_table = off;  off += round_up((size_t)RUN_CHUNK * sizeof(StepCoef), 256);
+    w.step_ctr = off;    off += 256;
     w.total = off;
     return w;
 }
@@ -278,6 +287,33 @@ int enqueue_force_kick_drift(double cv, double ck, double d2, float tag) {
     return COLATUS_OK;
 }
 
+void invalidate_graph() { g.graph_valid = false; }
+
+// One step with the coefficients of table row ctr[0] (integrate_kernels.cuh "table-driven variants"):
+// the same five launches as colatus_step, with step-independent arguments, on stream `st`.
+int enqueue_step_table(cudaStream_t st) {
+    const Workspace w = workspace_layout(g.n);
+    const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
+    int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
+    const unsigned blocks = (unsigned)((g.t_count + 255) / 256);
+    drift_table_kernel<<<blocks, 256, 0, st>>>(g.pos, g.vel, g.t_begin, g.t_count, table, ctr);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    int rc = run_forces(g.pos, g.n, g.t_begin, g.t_count, g.eps2, g.acc, false, st);
+    if (rc) return rc;
+    if (g.trace_k > 0) {
+        const int32_t *slot = reinterpret_cast<const int32_t *>(g.ws + w.trace_slot);
+        kick_drift_table_kernel<true><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, table, ctr,
+                                                              slot, g.ring, g.trace_k);
+    } else {
+        kick_drift_table_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, table, ctr,
+                                                               nullptr, nullptr, 0);
+    }
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
 int build_trace_map(const int32_t *idx_dev) {
     const Workspace w = workspace_layout(g.n);
     if (w.total > g.ws_bytes) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace too small for n=%lld", (long long)g.n);
@@ -325,12 +361,23 @@ int colatus_init(const colatus_config *cfg) {
     g.ev_used = 0;
     g.force_I = g.force_splits = 0;
     g.def_S = g.bg_rho = 0.0;
+    invalidate_graph();
     g.initialised = true;
     g.err[0] = 0;
     return COLATUS_OK;
 }
 
 void colatus_shutdown(void) {
+    if (g.graph_exec) cudaGraphExecDestroy(g.graph_exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    if (g.run_ev_in) cudaEventDestroy(g.run_ev_in);
+    if (g.run_ev_out) cudaEventDestroy(g.run_ev_out);
+    if (g.run_stream) cudaStreamDestroy(g.run_stream);
+    g.graph_exec = nullptr;
+    g.graph = nullptr;
+    g.run_ev_in = g.run_ev_out = nullptr;
+    g.run_stream = nullptr;
+    g.graph_valid = false;
     for (cudaEvent_t e : g.ev_pool) cudaEventDestroy(e);
     g.ev_pool.clear();
     g.ev_used = 0;
@@ -402,6 +449,7 @@ int colatus_upload(void *pos_mass_dev, void *vel_dev, void *acc_dev, int64_t n, 
     g.step = 0;
     g.trace_k = 0;
     g.uploaded = true;
+    invalidate_graph();
     return COLATUS_OK;
 }
 
@@ -411,6 +459,7 @@ int colatus_set_target_range(int64_t target_begin, int64_t target_count) {
     if (target_begin < 0 || target_count < 1 || target_begin + target_count > g.n)
         return fail(COLATUS_INVALID_ARG, "target range outside [0, n)");
     g.t_begin = target_begin;
+    invalidate_graph();
     g.t_count = target_count;
     return COLATUS_OK;
 }
@@ -488,6 +537,7 @@ int colatus_set_deformation(const double x_psi[3], double strength) {
         for (int i = 0; i < 3; ++i) g.def_x[i] = x_psi[i];
     }
     g.def_S = strength;
+    invalidate_graph();
     return COLATUS_OK;
 }
 
@@ -501,7 +551,102 @@ int colatus_set_background(const double centre[3], double rho_bar) {
         for (int i = 0; i < 3; ++i) g.bg_c[i] = centre[i];
     }
     g.bg_rho = rho_bar;
+    invalidate_graph();
     return COLATUS_OK;
+}
+
+int colatus_run(const colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph, double *a_end) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (n_steps < 1) return fail(COLATUS_INVALID_ARG, "n_steps < 1");
+    if (!std::isfinite(tau)) return fail(COLATUS_INVALID_ARG, "tau is not finite");
+    if (c && (!std::isfinite(a_start) || !(a_start > 0.0))) return fail(COLATUS_INVALID_ARG, "a_start must be > 0");
+    const Workspace w = workspace_layout(g.n);
+    if (w.total > g.ws_bytes) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace too small for n=%lld", (long long)g.n);
+
+    // the whole schedule first (eq. (2), host, double): nothing is enqueued if any step is invalid
+    std::vector<StepCoef> coef((size_t)n_steps);
+    double a = c ? a_start : 1.0;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        double a_mid = 1.0, H_mid = 0.0;                    // c == NULL: static background (reading G13)
+        if (c) {
+            a_mid = colatus_a_advance(c, a, 0.5 * tau);      // a, H at t_n + tau/2 (reading G3)
+            H_mid = colatus_hubble(c, a_mid);
+            a = colatus_a_advance(c, a_mid, 0.5 * tau);
+        }
+        double k[4];
+        int rc = colatus_step_coefficients(tau, a_mid, H_mid, k);
+        if (rc) return rc;
+        StepCoef &q = coef[(size_t)s];
+        q.d1 = (float)k[0];
+        q.cv = (float)k[1];
+        q.ck = (float)k[2];
+        q.d2 = (float)k[3];
+        q.tag = (float)a_mid;
+        q.ring_row = g.trace_k > 0 ? (int)((g.step + s) % g.trace_cap) : 0;
+        q.pad0 = q.pad1 = 0.f;
+    }
+
+    if (!g.run_stream) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&g.run_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaEventCreateWithFlags(&g.run_ev_in, cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&g.run_ev_out, cudaEventDisableTiming));
+    }
+    // the loop runs on the library's own stream (the caller's may be the legacy default stream, which
+    // cannot be captured), ordered after and before the resident stream by events
+    CUDA_TRY(cudaEventRecord(g.run_ev_in, g.stream));
+    CUDA_TRY(cudaStreamWaitEvent(g.run_stream, g.run_ev_in, 0));
+
+    const bool profile_was = g.profile;
+    g.profile = false;                                      // no event brackets inside a graph
+    int rc = COLATUS_OK;
+    if (use_graph && !g.graph_valid) {
+        if (g.graph_exec) cudaGraphExecDestroy(g.graph_exec);
+        if (g.graph) cudaGraphDestroy(g.graph);
+        g.graph_exec = nullptr;
+        g.graph = nullptr;
+        cudaError_t e = cudaStreamBeginCapture(g.run_stream, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+            const int64_t launches0 = g.launches;
+            rc = enqueue_step_table(g.run_stream);
+            g.launches = launches0;                         // captured, not launched
+            e = cudaStreamEndCapture(g.run_stream, &g.graph);
+            if (rc == COLATUS_OK && e == cudaSuccess) e = cudaGraphInstantiate(&g.graph_exec, g.graph, 0);
+        }
+        if (rc == COLATUS_OK && e != cudaSuccess)
+            rc = fail(COLATUS_CUDA_ERROR, "graph capture failed: %s", cudaGetErrorString(e));
+        g.graph_valid = rc == COLATUS_OK;
+    }
+    const Geometry geo = choose_geometry(g.n, g.t_count);
+    const int64_t per_step = 4 + (geo.splits > 1 ? 1 : 0) + ((g.def_S != 0.0 || g.bg_rho != 0.0) ? 1 : 0);
+    StepCoef *table = reinterpret_cast<StepCoef *>(g.ws + w.step_table);
+    int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
+    for (int64_t s0 = 0; rc == COLATUS_OK && s0 < n_steps; s0 += RUN_CHUNK) {
+        const int64_t m = n_steps - s0 < RUN_CHUNK ? n_steps - s0 : RUN_CHUNK;
+        cudaError_t e = cudaMemcpyAsync(table, coef.data() + s0, (size_t)m * sizeof(StepCoef), cudaMemcpyHostToDevice,
+                                        g.run_stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(ctr, 0, 2 * sizeof(int), g.run_stream);
+        if (e != cudaSuccess) {
+            rc = fail(COLATUS_CUDA_ERROR, "table upload failed: %s", cudaGetErrorString(e));
+            break;
+        }
+        for (int64_t s = 0; s < m && rc == COLATUS_OK; ++s) {
+            if (use_graph) {
+                e = cudaGraphLaunch(g.graph_exec, g.run_stream);
+                if (e != cudaSuccess) rc = fail(COLATUS_CUDA_ERROR, "cudaGraphLaunch failed: %s", cudaGetErrorString(e));
+                g.launches += per_step;
+            } else {
+                rc = enqueue_step_table(g.run_stream);
+            }
+            if (rc == COLATUS_OK) g.step++;
+        }
+    }
+    g.profile = profile_was;
+    // the resident stream waits for the loop whatever happened above, so later calls stay ordered
+    cudaEventRecord(g.run_ev_out, g.run_stream);
+    cudaStreamWaitEvent(g.stream, g.run_ev_out, 0);
+    if (rc == COLATUS_OK && a_end) *a_end = a;
+    return rc;
 }
 
 int colatus_drift(double d) {
@@ -523,6 +668,7 @@ int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_st
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
     if (k < 0) return fail(COLATUS_INVALID_ARG, "k < 0");
+    invalidate_graph();
     if (k == 0) {
         g.trace_k = 0;
         return COLATUS_OK;
@@ -711,6 +857,7 @@ int colatus_set_option(const char *name, int64_t value) {
     } else {
         return fail(COLATUS_INVALID_ARG, "unknown option %s", name);
     }
+    invalidate_graph();
     return COLATUS_OK;
 }
 

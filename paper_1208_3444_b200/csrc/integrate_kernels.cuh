@@ -52,6 +52,61 @@ kick_drift_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, const
     }
 }
 
+// ---- table-driven variants for colatus_run (CUDA-graph replay of a launch-bound step loop) ----------------
+// The per-step coefficients live in a device table; a device counter selects the row, so the five
+// kernels of a step have step-independent arguments and ONE captured graph is replayed every step.
+//   ctr[0] = step index the next drift uses;  ctr[1] = step index the kick-drift uses.
+// drift copies ctr[0] into ctr[1] (nobody reads ctr[1] while drift runs); kick-drift writes
+// ctr[0] = step + 1 (nobody reads ctr[0] while it runs).  Same arithmetic as the scalar kernels.
+struct StepCoef {
+    float d1, cv, ck, d2, tag;
+    int ring_row;       // (step % capacity) of this step's tracer row
+    float pad0, pad1;   // 32 B per row
+};
+
+__global__ void __launch_bounds__(256)
+drift_table_kernel(float4 *__restrict__ pos_mass, const float4 *__restrict__ vel, int64_t begin, int64_t count,
+                   const StepCoef *__restrict__ table, int *__restrict__ ctr) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = ctr[0];
+    if (i == 0) ctr[1] = s;
+    if (i >= count) return;
+    const float d = table[s].d1;
+    float4 p = pos_mass[begin + i];
+    const float4 v = vel[begin + i];
+    p.x = fmaf(d, v.x, p.x);
+    p.y = fmaf(d, v.y, p.y);
+    p.z = fmaf(d, v.z, p.z);
+    pos_mass[begin + i] = p;
+}
+
+template <bool TRACE>
+__global__ void __launch_bounds__(256)
+kick_drift_table_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, const float4 *__restrict__ acc,
+                        int64_t begin, int64_t count, const StepCoef *__restrict__ table, int *__restrict__ ctr,
+                        const int32_t *__restrict__ trace_slot, float4 *__restrict__ ring, int trace_k) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = ctr[1];
+    if (i == 0) ctr[0] = s + 1;
+    if (i >= count) return;
+    const StepCoef c = table[s];
+    float4 p = pos_mass[begin + i];
+    float4 v = vel[begin + i];
+    const float4 f = acc[i];
+    v.x = fmaf(c.ck, f.x, c.cv * v.x);
+    v.y = fmaf(c.ck, f.y, c.cv * v.y);
+    v.z = fmaf(c.ck, f.z, c.cv * v.z);
+    p.x = fmaf(c.d2, v.x, p.x);
+    p.y = fmaf(c.d2, v.y, p.y);
+    p.z = fmaf(c.d2, v.z, p.z);
+    vel[begin + i] = v;
+    pos_mass[begin + i] = p;
+    if (TRACE) {
+        const int32_t t = trace_slot[begin + i];
+        if (t >= 0) ring[(size_t)c.ring_row * trace_k + t] = make_float4(v.x, v.y, v.z, c.tag);
+    }
+}
+
 // External terms added to the force of eq. (1) for the target range (acc indexed from 0):
 //   eq. (10), PAPER.md:93 (reading G21):  F_k += S (x_psi - x_k) / (|x_k - x_psi|^2 + eps^2)^{3/2}
 //   background (reading G22):             F_k += B (x_k - centre),  B = (4 pi / 3) G rho_bar (host, double)

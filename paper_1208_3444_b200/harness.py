@@ -91,6 +91,10 @@ class Session:
                 a = B.colatus_a_advance(cosmo, a_mid, 0.5 * tau)
         return a
 
+    def run_native(self, cosmo, a_start: float, tau: float, steps: int, use_graph: bool = True):
+        """The same steps as `run`, in one colatus_run call (native loop, CUDA-graph replay)."""
+        return B.colatus_run(cosmo, a_start, tau, steps, use_graph)
+
     def download(self):
         pos = np.empty((self.n, 4), dtype=np.float32)
         vel = np.empty((self.n, 4), dtype=np.float32)

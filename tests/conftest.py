@@ -21,3 +21,16 @@ def pytest_collection_modifyitems(config, items):
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
+
+
+def record_parity(name, **values):
+    """Append measured GPU-vs-oracle errors to gpurun_out/parity_errors.jsonl (scratch; the numbers quoted in
+    DESIGN.md come from it).  Never influences a test outcome."""
+    import json
+    try:
+        d = os.path.join(ROOT, "gpurun_out")
+        os.makedirs(d, exist_ok=True)
+        with open(os.path.join(d, "parity_errors.jsonl"), "a") as f:
+            f.write(json.dumps({"case": name, **{k: float(v) for k, v in values.items()}}) + "\n")
+    except OSError:
+        pass

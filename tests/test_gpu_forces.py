@@ -12,6 +12,7 @@ pytestmark = pytest.mark.gpu
 import oracle  # noqa: E402
 from paper_1208_3444_b200 import binding as B  # noqa: E402
 from paper_1208_3444_b200 import inputs  # noqa: E402
+from conftest import record_parity  # noqa: E402
 
 MEDIAN_TOL = 1e-5
 MAX_TOL = 1e-4
@@ -39,6 +40,7 @@ def _check_config(session, index, n_targets=None):
     assert np.all(acc[:, 3] == 0.0)
     ref = oracle.forces(pm, cfg.eps2, 1.0, tg)
     med, mx = force_errors(acc[tg, :3], ref)
+    record_parity(f"forces config {index}", n=cfg.n, targets=len(tg), median_rel=med, max_over_rms=mx)
     assert med <= MEDIAN_TOL and mx <= MAX_TOL, (index, med, mx)
     # Newton's third law on the GPU result (P2): |sum m F| / sum m |F|
     m = pm[:, 3].astype(np.float64)

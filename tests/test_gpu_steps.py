@@ -13,6 +13,7 @@ pytestmark = pytest.mark.gpu
 import oracle  # noqa: E402
 from paper_1208_3444_b200 import binding as B  # noqa: E402
 from paper_1208_3444_b200 import inputs  # noqa: E402
+from conftest import record_parity  # noqa: E402
 
 POS_TOL = 1e-5
 
@@ -47,6 +48,7 @@ def test_ten_step_trajectory_parity(index):
     moved = np.linalg.norm(st.x - x0, axis=1).max()
     assert moved >= 100 * POS_TOL, f"vacuous: reference moved only {moved:g}"          # G16 guard
     err = np.linalg.norm(pos[:, :3].astype(np.float64) - st.x, axis=1).max()
+    record_parity(f"{steps}-step trajectory config {index}", n=cfg.n, max_dx_over_box=err, ref_moved=moved)
     assert err <= POS_TOL, (index, err)
     assert a_end == pytest.approx(ends[-1], rel=1e-9)
     assert np.array_equal(pos[:, 3], pm[:, 3])                                          # masses untouched
