@@ -52,6 +52,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-step-loops", action="store_true", help="skip the configs 1-3 steps/s side measurement")
     ap.add_argument("--n", type=int, default=0, help="override N (debug only; the reported workload is 2^20)")
     return ap.parse_args()
 
@@ -122,6 +123,42 @@ def oracle_sample_rate(pm, cfg, seconds_target=12.0, max_targets=65536):
     oracle.forces(pm, cfg.eps2, cfg.G, tg)
     dt = time.perf_counter() - t0
     return k * n / dt / 1e9, oracle.num_threads(), f"{k} seeded targets x {n} sources (config {cfg.index}), FP64, {dt:.1f} s"
+
+
+def step_loop_rates(device_index):
+    """Side measurement ("steps/s for configs 1-3, CUDA graph on/off"): whole leapfrog steps per
+    second of the small, launch-bound configurations through colatus_run with graph replay, the same kernels
+    launched one by one from the native loop, and colatus_step called per step from Python.  Device time by
+    CUDA events on the resident stream (colatus_run orders its own stream inside it); two repetitions, best."""
+    import torch
+    from paper_1208_3444_b200 import binding as B
+    from paper_1208_3444_b200 import inputs
+    from paper_1208_3444_b200.harness import Session
+    out = {}
+    for index, steps in ((1, 400), (2, 200), (3, 40)):
+        cfg, pm, vel = inputs.make_config(index)
+        row = {"n": cfg.n, "steps_timed": steps}
+        with Session(cfg.G, cfg.n, device=device_index) as s:
+            tau = 1e-3 * cfg.tau                       # tiny steps: the state stays near the initial one
+            for mode in ("graph", "launch", "python"):
+                best = None
+                for _ in range(3):                     # first repetition warms up / captures
+                    s.upload(pm, vel, cfg.eps2)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    torch.cuda.synchronize()
+                    e0.record()
+                    if mode == "python":
+                        s.run(cfg.cosmo, cfg.a_start, tau, steps)
+                    else:
+                        B.colatus_run(cfg.cosmo, cfg.a_start, tau, steps, mode == "graph")
+                    e1.record()
+                    torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1)
+                    best = ms if best is None else min(best, ms)
+                row[mode + "_steps_per_s"] = steps / (best * 1e-3)
+            row["graph_Ginteractions_per_s"] = row["graph_steps_per_s"] * float(cfg.n) ** 2 / 1e9
+        out[f"config{index}"] = row
+    return out
 
 
 def run_reference(args):
@@ -269,8 +306,12 @@ def run_native(args):
         v, cores, sample = oracle_sample_rate(pm, cfg)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
+    sess.close()
+    step_loops = None
+    if rank == 0 and world == 1 and not args.no_step_loops and not args.n:
+        step_loops = step_loop_rates(local_rank)
+
     if rank == 0:
-        geo = B.colatus_force_geometry(n, count)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
@@ -286,11 +327,11 @@ def run_native(args):
             "frac_fp32_peak": value * FLOP_PER_INTERACTION / 1e3 / (FP32_PEAK_TFLOPS * world),
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
             "gpu_launches": int(launches), "clocks": clocks,
+            "step_loops": step_loops,
             "diagnostics_last_step": {"M": diag[0], "T": diag[7]},
             "paper_context": "paper reports no timing; largest run 32^3 particles on a GTX680 (PAPER.md:23)",
         }
         print(json.dumps(line), flush=True)
-    sess.close()
     if world > 1:
         dist.destroy_process_group()
 
