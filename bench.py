@@ -53,6 +53,8 @@ def parse():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-step-loops", action="store_true", help="skip the configs 1-3 steps/s side measurement")
+    ap.add_argument("--config", type=int, default=WORKLOAD_CONFIG, choices=[4, 5],
+                    help="4 = N=2^20 (the reported workload, default); 5 = N=2^22 (the at-scale case of BASELINE.json)")
     ap.add_argument("--n", type=int, default=0, help="override N (debug only; the reported workload is 2^20)")
     return ap.parse_args()
 
@@ -167,7 +169,7 @@ def run_reference(args):
         return
     import oracle
     from paper_1208_3444_b200 import inputs
-    cfg, pm, _ = inputs.make_config(WORKLOAD_CONFIG, args.n or None)
+    cfg, pm, _ = inputs.make_config(args.config, args.n or None)
     n = pm.shape[0]
     k = 2048                                           # per-step sample: 2048 targets x N sources
     tg = inputs.sample_targets(cfg, k)
@@ -210,7 +212,7 @@ def run_native(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    cfg, pm, vel = inputs.make_config(WORKLOAD_CONFIG, args.n or None)
+    cfg, pm, vel = inputs.make_config(args.config, args.n or None)
     n = pm.shape[0]
     cosmo = inputs.Cosmology(H0=float(np.sqrt(8.0 * np.pi / 3.0)), Om_M=1.0)     # EdS, as config 1
     sess = Session(cfg.G, n, device=local_rank)
@@ -275,7 +277,7 @@ def run_native(args):
     k_ms = kernel_ms / max(kernel_launches, 1)
     achieved = FLOP_PER_INTERACTION * pairs_per_launch / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / FP32_PEAK_TFLOPS, "traffic": FORCE_KERNEL_DRAM_TRAFFIC_BYTES,
+                "frac": achieved / FP32_PEAK_TFLOPS, "traffic": FORCE_KERNEL_DRAM_TRAFFIC_BYTES if (n == 1 << 20 and world == 1) else None,
                 "kernel": "force_kernel<%d,%d,4,false,2>" % (geo["targets_per_thread"] // 2,
                                                              {6: 512, 4: 512, 2: 256}[geo["targets_per_thread"]]),
                 "kernel_ms": k_ms,
@@ -308,7 +310,7 @@ def run_native(args):
 
     sess.close()
     step_loops = None
-    if rank == 0 and world == 1 and not args.no_step_loops and not args.n:
+    if rank == 0 and world == 1 and not args.no_step_loops and not args.n and args.config == WORKLOAD_CONFIG:
         step_loops = step_loop_rates(local_rank)
 
     if rank == 0:
@@ -316,7 +318,7 @@ def run_native(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"config {cfg.index}: N={n}, 64 Gaussian clusters + 50% uniform background, "
+            "config": {"workload": f"config {cfg.index}: N={n}, {64 if cfg.index == 4 else 256} Gaussian clusters + 50% uniform background, "
                                    f"log-normal masses, eps={cfg.eps}; one full leapfrog step + diagnostics per step",
                        "n": n, "interactions_per_step": float(n) * n, "tracers": N_TRACERS,
                        "parallelism": "single GPU" if world == 1 else f"targets sharded over {world} GPUs, "

@@ -27,6 +27,7 @@
  *                      eqs. (3)-(5) as tau -> 0 at second order
  *   oracle_add_external P13 extra-body equivalence + two-body closed form (eq. 10),
  *                      linear closed form + homogeneous-sphere cancellation
+ *   oracle_forces + oracle_step  P16 cold homogeneous sphere vs the scalar shell recurrence
  *   oracle_splat       P14 brute-force counts, total = in-window particles
  *   oracle_trace_spectrum P15 sinusoid closed form, Parseval, numpy FFT
  * Unpinned: nothing in this file.  (Physical realism of config 2 against the
