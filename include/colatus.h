@@ -253,6 +253,13 @@ int      colatus_profile(int enable);
 int      colatus_profile_read(double *total_ms, int64_t *launches);
 int64_t  colatus_launch_count(void);
 
+/* Measures the plain FP32 FMA throughput of the device with a register-only loop (packed = 0: scalar
+ * FFMA; 1: FFMA2 / fma.rn.f32x2): the denominator of the "alu" roofline, which
+ * MEASURED_PEAKS.json does not carry.  *tflops = 2 flop x lane-FMAs / best of three timed launches
+ * (16 waves of 8 CTAs/SM, 8 independent chains per thread); *ms_out (may be NULL) = that launch's
+ * duration.  Runs on the default stream and synchronises. */
+int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out);
+
 /* Geometry the force path picked for n bodies / target_count targets on this device:
  * out[0] = targets per CTA, out[1] = target tiles, out[2] = source splits,
  * out[3] = sources per split (padded), out[4] = CTAs per SM, out[5] = SM count,

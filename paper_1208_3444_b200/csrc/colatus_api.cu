@@ -15,6 +15,7 @@
 #include "force_kernels.cuh"
 #include "integrate_kernels.cuh"
 #include "analysis_kernels.cuh"
+#include "calibrate_kernels.cuh"
 
 namespace {
 
@@ -825,6 +826,39 @@ int colatus_profile_read(double *total_ms, int64_t *launches) {
     *total_ms = sum;
     *launches = (int64_t)(g.ev_used / 2);
     g.ev_used = 0;
+    return COLATUS_OK;
+}
+
+int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!tflops) return fail(COLATUS_INVALID_ARG, "tflops is null");
+    if (workspace_layout(1).total > g.ws_bytes) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace too small");
+    float *sink = reinterpret_cast<float *>(g.ws);            // never written (see calibrate_kernels.cuh)
+    const int blocks = g.sm_count * 8 * 16;                    // 16 full waves of 8 CTAs/SM
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    float best = 0.f;
+    cudaError_t err = cudaSuccess;
+    for (int r = 0; r < 4 && err == cudaSuccess; ++r) {        // first repetition is the warm-up
+        cudaEventRecord(e0, nullptr);
+        if (packed)
+            calibrate_fma_kernel<1><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink);
+        else
+            calibrate_fma_kernel<0><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink);
+        cudaEventRecord(e1, nullptr);
+        err = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && (best == 0.f || ms < best)) best = ms;
+        g.launches++;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return fail(COLATUS_CUDA_ERROR, "calibration failed: %s", cudaGetErrorString(err));
+    const double lane_fma = (double)blocks * CAL_THREADS * (double)CAL_ITERS * CAL_CHAINS * 2.0;   // per launch
+    *tflops = 2.0 * lane_fma / ((double)best * 1e-3) / 1e12;
+    if (ms_out) *ms_out = best;
     return COLATUS_OK;
 }
 

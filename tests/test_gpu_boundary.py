@@ -91,3 +91,13 @@ def test_launch_count_and_geometry(session):
     assert geo["sm_count"] == 148 and geo["threads_per_cta"] == 256
     assert geo["target_tiles"] * geo["targets_per_cta"] >= 5000
     assert geo["source_splits"] * geo["sources_per_split"] >= 5000
+
+
+def test_calibrated_fp32_peak_is_near_the_derived_one(session):
+    """148 SMs x 128 lanes x 2 flop x clock.  The register-only loops must land within
+    a few percent of it at the clock the device actually runs (never above the max-clock figure)."""
+    for packed in (0, 1):
+        tflops, ms = B.colatus_calibrate_fp32(packed)
+        assert ms > 0
+        assert 0.80 * 74.45 <= tflops <= 1.01 * 74.45, (packed, tflops)
+    assert B.lib().colatus_calibrate_fp32(0, None, None) == B.INVALID_ARG
