@@ -113,12 +113,20 @@ Workspace workspace_layout(int64_t n_max) {
     return w;
 }
 
-// Pick (I, TJ) and the source split so that CTAs ~ k * (SMs * CTAs/SM) with little padding
-// (DESIGN.md "Launch geometry").
+// Pick the kernel variant (target pairs per thread, tile) and the source split by a cost model fitted to
+// a sweep of every (variant, split) at N = 4096 ... 262144 on the B200 (DESIGN.md 6.3 "Launch geometry";
+// rms error 2 %, picks within 0.7 % of the best measured geometry at every size):
+//   time ~ a_IP * IP * S * (per_sm + 0.1) + per_sm * c0
+// S = padded sources per split, per_sm = ceil(CTAs / SMs) (an SM works through its CTAs two at a time,
+// work-conserving, so what counts is CTAs per SM, not waves of resident slots), a_IP = time per source and
+// target pair of a CTA with the SM to itself, c0 = per-CTA prologue/epilogue.  Pure function of
+// (n, t_count, SM count): the geometry, and with it the summation order, is reproducible.
 Geometry choose_geometry(int64_t n, int64_t t_count) {
     static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 256}};   // (target pairs per thread, tile)
-    const int64_t slots = (int64_t)g.sm_count * g.ctas_per_sm;
+    static const double a_us[4] = {0.0, 0.0295, 0.0287, 0.0274};        // per source, per target pair
+    const double c0_us = 0.77, ramp = 0.096;
     Geometry best;
+    double best_cost = -1.0;
     for (int v = 0; v < 3; ++v) {
         const int IP = variants[v][0], TJ = variants[v][1];
         if (g.force_I && g.force_I != 2 * IP) continue;
@@ -126,17 +134,14 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
         const int64_t tiles_t = (t_count + per_cta - 1) / per_cta;
         const int64_t src_tiles = (n + TJ - 1) / TJ;
         const int64_t smax = src_tiles < MAX_SPLITS ? src_tiles : MAX_SPLITS;
-        if (!g.force_I && v < 2 && tiles_t * smax < slots) continue;   // too few CTAs: finer variant
-        double best_eff = -1.0;
         for (int64_t s = 1; s <= smax; ++s) {
             if (g.force_splits && s != g.force_splits && g.force_splits <= smax) continue;
             const int64_t tps = (src_tiles + s - 1) / s;
             const int64_t units = tiles_t * s;
-            const int64_t waves = (units + slots - 1) / slots;
-            double eff = (double)units / (double)(waves * slots) * (double)src_tiles / (double)(s * tps);
-            eff *= (double)tps / ((double)tps + 0.125);   // per-CTA prologue/epilogue
-            if (eff > best_eff * 1.002) {                 // prefer fewer splits on near ties
-                best_eff = eff;
+            const int64_t per_sm = (units + g.sm_count - 1) / g.sm_count;
+            const double cost = a_us[IP] * IP * (double)(tps * TJ) * ((double)per_sm + ramp) + (double)per_sm * c0_us;
+            if (best_cost < 0.0 || cost < best_cost * 0.998) {   // prefer earlier (fewer splits, more targets) on near ties
+                best_cost = cost;
                 best.IP = IP;
                 best.TJ = TJ;
                 best.tiles_t = tiles_t;
@@ -145,7 +150,6 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
                 best.n_pad = s * tps * TJ;
             }
         }
-        break;
     }
     return best;
 }
