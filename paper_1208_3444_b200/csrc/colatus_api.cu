@@ -37,6 +37,7 @@ struct Geometry {
 struct Workspace {     // byte offsets inside the caller's workspace
     size_t packed = 0, partials = 0, scratch_acc = 0, trace_slot = 0, diag = 0, stage_in = 0, stage_out = 0,
            step_table = 0, step_ctr = 0, total = 0;
+    static constexpr size_t mass_flag = 0;   // first 256 bytes of the workspace: fixed place for every n
 };
 
 struct Context {
@@ -63,6 +64,7 @@ struct Context {
     int64_t launches = 0;
     // tuning overrides (0 = automatic)
     int force_I = 0, force_splits = 0;
+    int generation = 0;   // equal-mass detection stamp (never 0: the flag word starts at 0)
     // external terms: eq. (10) source and mean-density background (0 = off)
     double def_S = 0.0, def_x[3] = {0, 0, 0}, bg_rho = 0.0, bg_c[3] = {0, 0, 0};
     // colatus_run: private capture stream, ordering events, cached one-step graph
@@ -99,7 +101,7 @@ Workspace workspace_layout(int64_t n_max) {
     Workspace w;
     const size_t n = (size_t)n_max;
     const size_t n_pad = round_up(n, (size_t)PAD_SOURCES) + (size_t)MAX_SPLITS * PAD_SOURCES;
-    size_t off = 0;
+    size_t off = 256;                        // [0, 256): mass_flag (zeroed by colatus_init)
     w.packed = off;      off += round_up(n_pad * 16, 256);
     w.partials = off;    off += round_up((size_t)MAX_SPLITS * n * 16, 256);
     w.scratch_acc = off; off += round_up(n * 16, 256);
@@ -157,7 +159,7 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
 template <int IP, int TJ, bool POT>
 cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
                                  int64_t t_count, float eps2, float scale, int final_out, float4 *out,
-                                 int64_t out_stride, cudaStream_t st) {
+                                 int64_t out_stride, const int *mass_flag, int generation, cudaStream_t st) {
     auto kern = force_kernel<IP, TJ, NSTAGES, POT, 2>;
     const size_t smem = force_smem_bytes<IP, TJ, NSTAGES, POT>();
     static bool attr_set = false;
@@ -168,24 +170,24 @@ cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, co
     }
     dim3 grid((unsigned)geo.tiles_t, (unsigned)geo.splits);
     kern<<<grid, FORCE_THREADS, smem, st>>>(pos_mass, packed, t_begin, t_count, geo.tiles_per_split, eps2, scale,
-                                            final_out, out, out_stride);
+                                            final_out, out, out_stride, mass_flag, generation);
     return cudaGetLastError();
 }
 
 template <bool POT>
 cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
                          int64_t t_count, float eps2, float scale, int final_out, float4 *out, int64_t out_stride,
-                         cudaStream_t st) {
+                         const int *mass_flag, int generation, cudaStream_t st) {
     switch (geo.IP) {
         case 3:
             return launch_force_variant<3, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
-                                                      final_out, out, out_stride, st);
+                                                      final_out, out, out_stride, mass_flag, generation, st);
         case 2:
             return launch_force_variant<2, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
-                                                     final_out, out, out_stride, st);
+                                                     final_out, out, out_stride, mass_flag, generation, st);
         default:
             return launch_force_variant<1, 256, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
-                                                     final_out, out, out_stride, st);
+                                                     final_out, out, out_stride, mass_flag, generation, st);
     }
 }
 
@@ -200,7 +202,13 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
     float4 *partials = reinterpret_cast<float4 *>(g.ws + w.partials);
 
-    stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed);
+    // equal-mass detection: a fresh generation per force evaluation; a body whose mass differs from body 0's
+    // stamps it into the flag, the force kernel compares (force_kernels.cuh)
+    int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
+    g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
+    const int generation = g.generation;
+    stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed,
+                                                                              mass_flag, generation);
     CUDA_TRY(cudaGetLastError());
     g.launches++;
 
@@ -221,9 +229,9 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         CUDA_TRY(cudaEventRecord(e0, st));
     }
     cudaError_t e = potential ? launch_force<true>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single, fout,
-                                                   t_count, st)
+                                                   t_count, mass_flag, generation, st)
                               : launch_force<false>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single,
-                                                    fout, t_count, st);
+                                                    fout, t_count, mass_flag, generation, st);
     CUDA_TRY(e);
     g.launches++;
     if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
@@ -357,8 +365,11 @@ int colatus_init(const colatus_config *cfg) {
     g.device = cfg->device;
     g.sm_count = prop.multiProcessorCount;
     g.ctas_per_sm = 2;
+    if (cfg->workspace_bytes < 256) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace smaller than 256 bytes");
+    CUDA_TRY(cudaMemset(cfg->workspace_dev, 0, 256));        // mass_flag and friends
     g.ws = static_cast<unsigned char *>(cfg->workspace_dev);
     g.ws_bytes = cfg->workspace_bytes;
+    g.generation = 0;
     g.uploaded = false;
     g.trace_k = 0;
     g.step = 0;
@@ -837,7 +848,7 @@ int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out) {
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!tflops) return fail(COLATUS_INVALID_ARG, "tflops is null");
     if (workspace_layout(1).total > g.ws_bytes) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace too small");
-    float *sink = reinterpret_cast<float *>(g.ws);            // never written (see calibrate_kernels.cuh)
+    float *sink = reinterpret_cast<float *>(g.ws + 128);      // never written (see calibrate_kernels.cuh)
     const int blocks = g.sm_count * 8 * 16;                    // 16 full waves of 8 CTAs/SM
     cudaEvent_t e0, e1;
     CUDA_TRY(cudaEventCreate(&e0));

@@ -170,3 +170,63 @@ def test_closed_form_three_body_on_gpu(session, golden_dir):
                 rows[t[0]] = [float(Fraction(s)) for s in t[1:]]
     for i, body in enumerate("ABC"):
         assert np.allclose(out[i, :3], rows[body], rtol=2e-6, atol=1e-8)
+
+
+# ---- equal-mass loop (11 packed ops per pair-interaction): taken iff every mass equals body 0's ----------
+@pytest.mark.parametrize("n", [2, 257, 1025, 4099, 20000])
+@pytest.mark.parametrize("variant", [0, 2, 4, 6])
+def test_equal_mass_loop_ragged_sizes_all_variants(session, n, variant):
+    """Equal masses (configs 1-3, every cosmological run) take the loop without the per-source mass
+    multiply; the common mass is applied to the finished sums.  Same tolerances, potential included."""
+    rng = np.random.Generator(np.random.PCG64(300 + n))
+    pm = np.empty((n, 4), dtype=np.float32)
+    pm[:, :3] = rng.random((n, 3))
+    pm[:, 3] = np.float32(0.37 / n)
+    eps2 = np.float32(0.02 ** 2)
+    B.colatus_set_option("targets_per_thread", variant)
+    try:
+        out = session.forces(pm, eps2, potential=True).cpu().numpy()
+    finally:
+        B.colatus_set_option("targets_per_thread", 0)
+    ref, phi = oracle.forces(pm, eps2, 1.0, potential=True)
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (n, variant, med, mx)
+    assert np.allclose(out[:, 3], phi, rtol=2e-5, atol=0)
+
+
+def test_one_different_mass_switches_to_the_general_loop(session):
+    """A single body with another mass (first, middle or last; also mass 0 and a tiny difference of one ulp)
+    must be honoured: the result follows the oracle for the actual masses, not for equal ones."""
+    cfg, pm0, _ = inputs.make_config(1)
+    base = oracle.forces(pm0, cfg.eps2, 1.0)
+    for where, factor in ((0, 3.0), (2048, 0.0), (4095, 50.0), (1234, None)):
+        pm = pm0.copy()
+        pm[where, 3] = np.nextafter(pm[where, 3], np.float32(1.0)) if factor is None else pm[where, 3] * factor
+        out = session.forces(pm, cfg.eps2).cpu().numpy()
+        ref = oracle.forces(pm, cfg.eps2, 1.0)
+        med, mx = force_errors(out[:, :3], ref)
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL, (where, factor, med, mx)
+        if factor not in (None,):
+            # the changed mass matters at the 1e-4 level somewhere, so a kernel that ignored it would fail above
+            assert np.abs(ref - base).max() > 1e3 * MAX_TOL * np.sqrt((base ** 2).sum(1).mean()) or factor == 3.0
+    # and back to equal masses: bitwise the same as before the excursion (the flag is per evaluation)
+    a = session.forces(pm0, cfg.eps2).cpu().numpy()
+    session.forces(pm, cfg.eps2)
+    b = session.forces(pm0, cfg.eps2).cpu().numpy()
+    assert np.array_equal(a, b)
+
+
+def test_all_zero_and_nan_masses(session):
+    cfg, pm, _ = inputs.make_config(1)
+    z = pm.copy()
+    z[:, 3] = 0.0                                        # equal (zero) masses: exact zeros, no NaN
+    out = session.forces(z, cfg.eps2, potential=True).cpu().numpy()
+    assert np.all(out == 0.0)
+    q = pm.copy()
+    q[7, 3] = np.nan                                     # NaN compares unequal -> general loop -> NaN out (no error)
+    out = session.forces(q, cfg.eps2).cpu().numpy()
+    assert np.isnan(out[:, :3]).all(axis=1).sum() >= cfg.n - 1
+    q = pm.copy()
+    q[0, 3] = np.nan                                     # NaN in body 0: every comparison is unequal
+    out = session.forces(q, cfg.eps2).cpu().numpy()
+    assert np.isnan(out[1:, :3]).all()

@@ -123,3 +123,30 @@ def test_run_argument_validation_enqueues_nothing():
                 B.colatus_run(*args)
         pos, v = s.download()
         assert np.array_equal(pos, pm) and np.array_equal(v, vel) and s.diagnostics(1.0)[12] == 0
+
+
+def test_cached_graph_honours_a_mass_change_between_runs():
+    """The equal-mass decision is taken on the device at every force evaluation (stage kernel stamps a flag),
+    so a graph captured while all masses were equal stays correct after the caller edits a mass in its
+    resident buffer -- bitwise the same as per-step colatus_step calls on the same sequence."""
+    import torch
+    cfg, pm, vel = inputs.make_config(1)
+    outs = []
+    for native in (True, False):
+        from paper_1208_3444_b200.harness import Session
+        with Session(cfg.G, cfg.n) as s:
+            s.upload(pm, vel, cfg.eps2)
+            step = (lambda k: s.run_native(None, 1.0, 1e-3, k)) if native else (lambda k: s.run(None, 1.0, 1e-3, k))
+            step(3)
+            torch.cuda.synchronize()
+            s.pos[100, 3] *= 40.0                      # the caller owns the buffer
+            step(3)
+            s.pos[100, 3] /= 40.0
+            step(2)
+            outs.append(s.download())
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+    for k in range(8):
+        st.m[100] = pm[100, 3] * (40.0 if 3 <= k < 6 else 1.0)
+        st.step(1e-3, 1.0, 0.0)
+    assert np.linalg.norm(outs[0][0][:, :3].astype(np.float64) - st.x, axis=1).max() <= POS_TOL
