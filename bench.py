@@ -38,7 +38,7 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-kernel launch at N = 2^20 from the
 # `ncu --set full` capture summarised in profiles/ (None until that capture exists).
-FORCE_KERNEL_DRAM_TRAFFIC_BYTES = 222765312     # profiles/r01_force_kernel_ncu_full.txt
+FORCE_KERNEL_DRAM_TRAFFIC_BYTES = 130877184     # profiles/r01_force_kernel_ncu_full.txt
 METRIC = "Ginteractions/s softened direct-sum gravity at N=2^20; % of FP32 FMA peak"
 UNIT = "Ginteractions/s"
 BENCH_TAU = 1.0e-6                         # step size of the bench steps (EdS background from a = 0.02)
