@@ -150,6 +150,12 @@ int colatus_step_coeffs(double d1, double cv, double ck, double d2);
  * Asynchronous. */
 int colatus_run(const struct colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph,
                 double *a_end);
+/* The same loop with the symplectic operators of eq. (9): per step the coefficients of
+ * colatus_symplectic_coefficients (drift and kick integrals along eq. (2), FP64 on the host); the resident
+ * "velocity" array holds w = a^2 v; tracer tag = a(t + tau).  c == NULL reduces to the static leapfrog.
+ * Bitwise identical to n_steps calls of colatus_step_symplectic. */
+int colatus_run_symplectic(const struct colatus_cosmo *c, double a_start, double tau, int64_t n_steps,
+                           int use_graph, double *a_end);
 
 /* ---- eq. (9): symplectic drift-kick-drift (reading G11) ---------------
  * The resident "velocity" array then holds w = p/m = a^2 v (canonical momentum per unit mass).

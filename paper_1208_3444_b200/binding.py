@@ -53,6 +53,7 @@ SIGNATURES = {
     "colatus_step_coefficients": (c_int, [c_double, c_double, c_double, POINTER(c_double)]),
     "colatus_step_coeffs": (c_int, [c_double, c_double, c_double, c_double]),
     "colatus_run": (c_int, [POINTER(colatus_cosmo), c_double, c_double, c_int64, c_int, POINTER(c_double)]),
+    "colatus_run_symplectic": (c_int, [POINTER(colatus_cosmo), c_double, c_double, c_int64, c_int, POINTER(c_double)]),
     "colatus_symplectic_coefficients": (c_int, [POINTER(colatus_cosmo), c_double, c_double, POINTER(c_double)]),
     "colatus_step_symplectic": (c_int, [POINTER(colatus_cosmo), c_double, c_double, POINTER(c_double)]),
     "colatus_set_deformation": (c_int, [POINTER(c_double), c_double]),
@@ -201,6 +202,15 @@ def colatus_run(cosmo, a_start, tau, n_steps, use_graph=True):
     a_end = c_double(0.0)
     cp = None if cosmo is None else ctypes.byref(_cosmo(cosmo))
     _check(lib().colatus_run(cp, float(a_start), float(tau), int(n_steps), int(bool(use_graph)), ctypes.byref(a_end)))
+    return a_end.value
+
+
+def colatus_run_symplectic(cosmo, a_start, tau, n_steps, use_graph=True):
+    """n_steps symplectic steps of eq. (9) in one native call (CUDA-graph replay).  Returns a_end."""
+    a_end = c_double(0.0)
+    cp = None if cosmo is None else ctypes.byref(_cosmo(cosmo))
+    _check(lib().colatus_run_symplectic(cp, float(a_start), float(tau), int(n_steps), int(bool(use_graph)),
+                                        ctypes.byref(a_end)))
     return a_end.value
 
 

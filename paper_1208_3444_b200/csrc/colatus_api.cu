@@ -571,7 +571,8 @@ int colatus_set_background(const double centre[3], double rho_bar) {
     return COLATUS_OK;
 }
 
-int colatus_run(const colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph, double *a_end) {
+static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph, double *a_end,
+                     bool symplectic) {
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
     if (n_steps < 1) return fail(COLATUS_INVALID_ARG, "n_steps < 1");
@@ -584,21 +585,31 @@ int colatus_run(const colatus_cosmo *c, double a_start, double tau, int64_t n_st
     std::vector<StepCoef> coef((size_t)n_steps);
     double a = c ? a_start : 1.0;
     for (int64_t s = 0; s < n_steps; ++s) {
-        double a_mid = 1.0, H_mid = 0.0;                    // c == NULL: static background (reading G13)
-        if (c) {
-            a_mid = colatus_a_advance(c, a, 0.5 * tau);      // a, H at t_n + tau/2 (reading G3)
-            H_mid = colatus_hubble(c, a_mid);
-            a = colatus_a_advance(c, a_mid, 0.5 * tau);
+        double k[4], tag;
+        if (symplectic && c) {                               // eq. (9): drift / kick integrals along eq. (2)
+            double q[5];
+            int rc = colatus_symplectic_coefficients(c, a, tau, q);
+            if (rc) return rc;
+            k[0] = q[0]; k[1] = q[1]; k[2] = q[2]; k[3] = q[3];
+            a = q[4];
+            tag = a;                                         // a(t + tau), as colatus_step_symplectic
+        } else {
+            double a_mid = 1.0, H_mid = 0.0;                 // c == NULL: static background (reading G13)
+            if (c) {
+                a_mid = colatus_a_advance(c, a, 0.5 * tau);  // a, H at t_n + tau/2 (reading G3)
+                H_mid = colatus_hubble(c, a_mid);
+                a = colatus_a_advance(c, a_mid, 0.5 * tau);
+            }
+            int rc = colatus_step_coefficients(tau, a_mid, H_mid, k);
+            if (rc) return rc;
+            tag = a_mid;
         }
-        double k[4];
-        int rc = colatus_step_coefficients(tau, a_mid, H_mid, k);
-        if (rc) return rc;
         StepCoef &q = coef[(size_t)s];
         q.d1 = (float)k[0];
         q.cv = (float)k[1];
         q.ck = (float)k[2];
         q.d2 = (float)k[3];
-        q.tag = (float)a_mid;
+        q.tag = (float)tag;
         q.ring_row = g.trace_k > 0 ? (int)((g.step + s) % g.trace_cap) : 0;
         q.pad0 = q.pad1 = 0.f;
     }
@@ -663,6 +674,15 @@ int colatus_run(const colatus_cosmo *c, double a_start, double tau, int64_t n_st
     cudaStreamWaitEvent(g.stream, g.run_ev_out, 0);
     if (rc == COLATUS_OK && a_end) *a_end = a;
     return rc;
+}
+
+int colatus_run(const colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph, double *a_end) {
+    return run_steps(c, a_start, tau, n_steps, use_graph, a_end, false);
+}
+
+int colatus_run_symplectic(const colatus_cosmo *c, double a_start, double tau, int64_t n_steps, int use_graph,
+                           double *a_end) {
+    return run_steps(c, a_start, tau, n_steps, use_graph, a_end, true);
 }
 
 int colatus_drift(double d) {
@@ -792,7 +812,7 @@ int colatus_diagnostics(double a, int with_potential, double out[16]) {
                                                              with_potential ? scratch : nullptr, g.t_count, partial);
     CUDA_TRY(cudaGetLastError());
     double *final_dev = partial + (size_t)DIAG_BLOCKS_MAX * DIAG_Q;
-    diagnostics_final_kernel<<<1, 32, 0, g.stream>>>(partial, blocks, final_dev);
+    diagnostics_final_kernel<<<1, DIAG_Q * 32, 0, g.stream>>>(partial, blocks, final_dev);
     CUDA_TRY(cudaGetLastError());
     g.launches += 2;
     double q[DIAG_Q];

@@ -195,13 +195,15 @@ __global__ void __launch_bounds__(256) diagnostics_partial_kernel(const float4 *
     }
 }
 
-__global__ void diagnostics_final_kernel(const double *__restrict__ partial, int blocks, double *__restrict__ out) {
-    const int c = threadIdx.x;
-    if (c < DIAG_Q) {
-        double s = 0.0;
-        for (int b = 0; b < blocks; ++b) s += partial[(size_t)b * DIAG_Q + c];
-        out[c] = s;
-    }
+// One warp per quantity: lane l adds partials l, l+32, ... in order, then a fixed xor-shuffle tree -- the
+// summation order depends only on `blocks`, so the result is reproducible.  Launch with DIAG_Q warps.
+__global__ void __launch_bounds__(DIAG_Q * 32)
+diagnostics_final_kernel(const double *__restrict__ partial, int blocks, double *__restrict__ out) {
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double s = 0.0;
+    for (int b = lane; b < blocks; b += 32) s += partial[(size_t)b * DIAG_Q + c];
+    s = warp_sum(s);
+    if (lane == 0) out[c] = s;
 }
 
 }  // namespace colatus

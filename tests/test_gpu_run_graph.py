@@ -150,3 +150,36 @@ def test_cached_graph_honours_a_mass_change_between_runs():
         st.m[100] = pm[100, 3] * (40.0 if 3 <= k < 6 else 1.0)
         st.step(1e-3, 1.0, 0.0)
     assert np.linalg.norm(outs[0][0][:, :3].astype(np.float64) - st.x, axis=1).max() <= POS_TOL
+
+
+@pytest.mark.parametrize("use_graph", [True, False])
+def test_run_symplectic_equals_step_symplectic_loop_bitwise(use_graph):
+    """Eq. (9) in the native loop: same coefficients, same kernels as colatus_step_symplectic per step."""
+    cfg, pm, vel = inputs.make_config(1)
+    rng = np.random.Generator(np.random.PCG64(21))
+    w0 = vel.copy()
+    w0[:, :3] = (cfg.a_start ** 2) * 0.05 * rng.standard_normal((cfg.n, 3)).astype(np.float32)
+    tr = np.arange(0, cfg.n, 256, dtype=np.int32)
+    outs = []
+    from paper_1208_3444_b200.harness import Session
+    for native in (False, True):
+        with Session(cfg.G, cfg.n) as s:
+            s.upload(pm, w0, cfg.eps2)
+            s.trace(tr, 4)
+            a = cfg.a_start
+            if native:
+                a = B.colatus_run_symplectic(cfg.cosmo, a, cfg.tau, 6, use_graph)
+            else:
+                for _ in range(6):
+                    a = B.colatus_step_symplectic(cfg.cosmo, a, cfg.tau)
+            pos, w = s.download()
+            outs.append((a, pos, w, s.ring.cpu().numpy()))
+    assert outs[0][0] == outs[1][0]
+    for x, y in zip(outs[0][1:], outs[1][1:]):
+        assert np.array_equal(x, y)
+    st = oracle.State(pm, w0, cfg.eps2, cfg.G)
+    a_ref = cfg.a_start
+    for _ in range(6):
+        a_ref = st.step_symplectic(cfg.cosmo, a_ref, cfg.tau)
+    assert outs[1][0] == pytest.approx(a_ref, rel=1e-9)
+    assert np.linalg.norm(outs[1][1][:, :3].astype(np.float64) - st.x, axis=1).max() <= POS_TOL
