@@ -64,6 +64,7 @@ struct Context {
     int64_t launches = 0;
     // tuning overrides (0 = automatic)
     int force_I = 0, force_splits = 0;
+    int init_epoch = 0;   // counts colatus_init calls
     int generation = 0;   // equal-mass detection stamp (never 0: the flag word starts at 0)
     // external terms: eq. (10) source and mean-density background (0 = off)
     double def_S = 0.0, def_x[3] = {0, 0, 0}, bg_rho = 0.0, bg_c[3] = {0, 0, 0};
@@ -162,11 +163,11 @@ cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, co
                                  int64_t out_stride, const int *mass_flag, int generation, cudaStream_t st) {
     auto kern = force_kernel<IP, TJ, NSTAGES, POT, 2>;
     const size_t smem = force_smem_bytes<IP, TJ, NSTAGES, POT>();
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int attr_epoch = 0;            // function attributes are per device: set again after every colatus_init
+    if (attr_epoch != g.init_epoch) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_epoch = g.init_epoch;
     }
     dim3 grid((unsigned)geo.tiles_t, (unsigned)geo.splits);
     kern<<<grid, FORCE_THREADS, smem, st>>>(pos_mass, packed, t_begin, t_count, geo.tiles_per_split, eps2, scale,
@@ -370,6 +371,7 @@ int colatus_init(const colatus_config *cfg) {
     g.ws = static_cast<unsigned char *>(cfg->workspace_dev);
     g.ws_bytes = cfg->workspace_bytes;
     g.generation = 0;
+    g.init_epoch++;
     g.uploaded = false;
     g.trace_k = 0;
     g.step = 0;

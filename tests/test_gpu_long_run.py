@@ -93,3 +93,46 @@ def test_config2_shaped_run_statistics():
     # the first 10 recorded steps still agree sample by sample
     vr = np.sqrt((rows_ref[:10, :, :3].astype(np.float64) ** 2).sum(2).mean())
     assert np.abs(rows_gpu[:10, :, :3] - rows_ref[:10, :, :3]).max() <= 2e-4 * vr
+
+
+def test_config3_shaped_cold_collapse_energy_and_virial():
+    """Config 3's own long run (reading G13/G20): Plummer sphere + 30 % background, cold start, static
+    background, 100 steps of tau = 1e-3 through maximum compression (near step 50) to a virialised state --
+    at N = 8192 so the oracle follows it in seconds.  Static limit: T + W is conserved by the flow, so the
+    GPU run is held to an absolute energy budget, and T, W are compared with the oracle's."""
+    from paper_1208_3444_b200.harness import Session
+    cfg, pm, vel = inputs.make_config(3, 8192)
+    steps, every = 100, 10
+    gpu = []
+    with Session(cfg.G, cfg.n) as s:
+        s.upload(pm, vel, cfg.eps2)
+        d = s.diagnostics(1.0, with_potential=True)
+        gpu.append((d[7], d[8]))
+        for _ in range(steps // every):
+            s.run_native(None, 1.0, cfg.tau, every)
+            d = s.diagnostics(1.0, with_potential=True)
+            gpu.append((d[7], d[8]))
+            assert np.abs(d[1:4]).max() <= 1e-5 * np.sqrt(2 * d[7] * d[0] + 1e-30) + 1e-9     # sum m v stays ~0
+    st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+    d = st.diagnostics(1.0, with_potential=True)
+    ref = [(d[7], d[8])]
+    for n in range(steps):
+        st.step(cfg.tau, 1.0, 0.0)
+        if (n + 1) % every == 0:
+            d = st.diagnostics(1.0, with_potential=True)
+            ref.append((d[7], d[8]))
+    E0 = ref[0][0] + ref[0][1]
+    assert gpu[0][0] == 0.0 and gpu[0][1] == pytest.approx(ref[0][1], rel=1e-6)
+    drift_gpu = max(abs(T + W - E0) / abs(E0) for T, W in gpu)
+    drift_ref = max(abs(T + W - E0) / abs(E0) for T, W in ref)
+    worst = 0.0
+    for k, ((Tg, Wg), (Tr, Wr)) in enumerate(zip(gpu, ref)):
+        if k == 0:
+            continue
+        tol = 1e-3 if k <= 3 else 1e-2                    # measured 5.5e-5 over the whole run
+        worst = max(worst, abs(Tg - Tr) / Tr, abs(Wg - Wr) / abs(Wr))
+        assert abs(Tg - Tr) <= tol * Tr and abs(Wg - Wr) <= tol * abs(Wr), (k * every, Tg, Tr, Wg, Wr)
+    record_parity("100-step config-3-shaped run (N=8192)", energy_drift_gpu=drift_gpu, energy_drift_oracle=drift_ref,
+                  worst_rel_T_or_W=worst)
+    assert drift_gpu <= max(2.0 * drift_ref, 0.02)
+    assert max(T for T, _ in ref) > 0.5 * abs(ref[0][1])   # it did collapse: T reaches the scale of |W0|
