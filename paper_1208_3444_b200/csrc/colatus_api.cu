@@ -21,7 +21,7 @@ namespace {
 
 using namespace colatus;
 
-constexpr int MAX_SPLITS = 16;        // source splits (partials kept in the workspace)
+constexpr int MAX_SPLITS = REDUCE_MAX_SPLITS;   // source splits (partials kept in the workspace)
 constexpr int NSTAGES = 4;            // shared-memory ring depth
 constexpr int DIAG_BLOCKS_MAX = 1024;
 constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
@@ -74,6 +74,7 @@ struct Context {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
     bool graph_valid = false;
+    int64_t graph_launches = 0;
     char err[512] = "";
 };
 
@@ -193,8 +194,16 @@ cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const floa
 }
 
 // stage + force (+ reduce): the whole of step a3.  No validation here.
+// `fused` (whole-range steps only): the staging pass also applies the drift of eq. (3) to the resident
+// positions (drift_stage_kernel), and the partial-sum reduction is left to the caller's fused
+// reduce-kick-drift kernel (*deferred_splits = number of partials to add, 0 if `out` is already final).
+struct FusedStep {
+    StepSrc src;
+    int deferred_splits = 0;
+};
+
 int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2, float4 *out,
-               bool potential, cudaStream_t st) {
+               bool potential, cudaStream_t st, FusedStep *fused = nullptr) {
     const Workspace w = workspace_layout(n);
     if (w.total > g.ws_bytes)
         return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
@@ -208,8 +217,12 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
     g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
     const int generation = g.generation;
-    stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed,
-                                                                              mass_flag, generation);
+    if (fused)
+        drift_stage_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(g.pos, g.vel, n, geo.n_pad, packed,
+                                                                                mass_flag, generation, fused->src);
+    else
+        stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed,
+                                                                                  mass_flag, generation);
     CUDA_TRY(cudaGetLastError());
     g.launches++;
 
@@ -237,6 +250,10 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     g.launches++;
     if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
 
+    if (fused) {
+        fused->deferred_splits = single ? 0 : geo.splits;
+        return COLATUS_OK;                      // no external terms in fused steps (checked by the caller)
+    }
     if (!single) {
         const unsigned blocks = (unsigned)((t_count + 255) / 256);
         if (potential)
@@ -301,6 +318,61 @@ int enqueue_force_kick_drift(double cv, double ck, double d2, float tag) {
     return COLATUS_OK;
 }
 
+// Whole-range step without external terms: three launches (drift+stage, force, reduce+kick+drift).
+bool can_fuse_step() { return g.t_begin == 0 && g.t_count == g.n && g.def_S == 0.0 && g.bg_rho == 0.0; }
+
+int enqueue_step_fused(StepSrc src, cudaStream_t st) {
+    FusedStep f;
+    f.src = src;
+    if (g.trace_k > 0 && !src.table) f.src.ring_row = (int)(g.step % g.trace_cap);
+    int rc = run_forces(g.pos, g.n, 0, g.n, g.eps2, g.acc, false, st, &f);
+    if (rc) return rc;
+    const Workspace w = workspace_layout(g.n);
+    const unsigned blocks = (unsigned)((g.n + 255) / 256);
+    const int32_t *slot = reinterpret_cast<const int32_t *>(g.ws + w.trace_slot);
+    const float4 *partials = reinterpret_cast<const float4 *>(g.ws + w.partials);
+    if (f.deferred_splits > 0) {
+        if (g.trace_k > 0)
+            reduce_kick_drift_kernel<true><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, partials, g.n, f.deferred_splits,
+                                                                   g.n, (float)g.G, f.src, slot, g.ring, g.trace_k);
+        else
+            reduce_kick_drift_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, partials, g.n,
+                                                                    f.deferred_splits, g.n, (float)g.G, f.src, nullptr,
+                                                                    nullptr, 0);
+    } else if (src.table) {                      // single split: acc is final, plain kick-drift
+        if (g.trace_k > 0)
+            kick_drift_table_kernel<true><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, 0, g.n, src.table, src.ctr, slot,
+                                                                  g.ring, g.trace_k);
+        else
+            kick_drift_table_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, 0, g.n, src.table, src.ctr,
+                                                                   nullptr, nullptr, 0);
+    } else {
+        float4 *row = g.trace_k > 0 ? g.ring + (size_t)f.src.ring_row * g.trace_k : nullptr;
+        if (g.trace_k > 0)
+            kick_drift_kernel<true><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, 0, g.n, src.cv, src.ck, src.d2, slot,
+                                                            row, src.tag);
+        else
+            kick_drift_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, 0, g.n, src.cv, src.ck, src.d2,
+                                                             nullptr, nullptr, src.tag);
+    }
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
+// One step with scalar coefficients on the resident stream: fused when possible, else the five launches.
+int enqueue_step_scalar(double d1, double cv, double ck, double d2, float tag) {
+    if (can_fuse_step()) {
+        StepSrc src{nullptr, nullptr, (float)d1, (float)cv, (float)ck, (float)d2, tag, 0};
+        int rc = enqueue_step_fused(src, g.stream);
+        if (rc == COLATUS_OK) g.step++;
+        return rc;
+    }
+    int rc = enqueue_drift(d1);
+    if (rc) return rc;
+    return enqueue_force_kick_drift(cv, ck, d2, tag);
+}
+
 void invalidate_graph() { g.graph_valid = false; }
 
 // One step with the coefficients of table row ctr[0] (integrate_kernels.cuh "table-driven variants"):
@@ -309,6 +381,10 @@ int enqueue_step_table(cudaStream_t st) {
     const Workspace w = workspace_layout(g.n);
     const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
     int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
+    if (can_fuse_step()) {
+        StepSrc src{table, ctr, 0.f, 0.f, 0.f, 0.f, 0.f, 0};
+        return enqueue_step_fused(src, st);
+    }
     const unsigned blocks = (unsigned)((g.t_count + 255) / 256);
     drift_table_kernel<<<blocks, 256, 0, st>>>(g.pos, g.vel, g.t_begin, g.t_count, table, ctr);
     CUDA_TRY(cudaGetLastError());
@@ -487,9 +563,7 @@ int colatus_step_coeffs(double d1, double cv, double ck, double d2) {
     if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
     if (!std::isfinite(d1) || !std::isfinite(cv) || !std::isfinite(ck) || !std::isfinite(d2))
         return fail(COLATUS_INVALID_ARG, "non-finite step coefficient");
-    int rc = enqueue_drift(d1);
-    if (rc) return rc;
-    return enqueue_force_kick_drift(cv, ck, d2, 0.f);
+    return enqueue_step_scalar(d1, cv, ck, d2, 0.f);
 }
 
 int colatus_step_coefficients(double tau, double a, double H, double out[4]) {
@@ -511,9 +585,7 @@ int colatus_step(double tau, double a, double H) {
     double c[4];
     int rc = colatus_step_coefficients(tau, a, H, c);
     if (rc) return rc;
-    rc = enqueue_drift(c[0]);                                            // eq. (3)
-    if (rc) return rc;
-    return enqueue_force_kick_drift(c[1], c[2], c[3], (float)a);         // eqs. (1), (4), (5)
+    return enqueue_step_scalar(c[0], c[1], c[2], c[3], (float)a);        // eqs. (3), (1), (4), (5)
 }
 
 int colatus_symplectic_coefficients(const colatus_cosmo *c, double a0, double tau, double out[5]) {
@@ -537,9 +609,7 @@ int colatus_step_symplectic(const colatus_cosmo *c, double a0, double tau, doubl
     double k[5];
     int rc = colatus_symplectic_coefficients(c, a0, tau, k);
     if (rc) return rc;
-    rc = enqueue_drift(k[0]);
-    if (rc) return rc;
-    rc = enqueue_force_kick_drift(k[1], k[2], k[3], (float)k[4]);
+    rc = enqueue_step_scalar(k[0], k[1], k[2], k[3], (float)k[4]);
     if (rc) return rc;
     if (a_end) *a_end = k[4];
     return COLATUS_OK;
@@ -638,6 +708,7 @@ static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t
         if (e == cudaSuccess) {
             const int64_t launches0 = g.launches;
             rc = enqueue_step_table(g.run_stream);
+            g.graph_launches = g.launches - launches0;      // kernels per replay
             g.launches = launches0;                         // captured, not launched
             e = cudaStreamEndCapture(g.run_stream, &g.graph);
             if (rc == COLATUS_OK && e == cudaSuccess) e = cudaGraphInstantiate(&g.graph_exec, g.graph, 0);
@@ -646,8 +717,6 @@ static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t
             rc = fail(COLATUS_CUDA_ERROR, "graph capture failed: %s", cudaGetErrorString(e));
         g.graph_valid = rc == COLATUS_OK;
     }
-    const Geometry geo = choose_geometry(g.n, g.t_count);
-    const int64_t per_step = 4 + (geo.splits > 1 ? 1 : 0) + ((g.def_S != 0.0 || g.bg_rho != 0.0) ? 1 : 0);
     StepCoef *table = reinterpret_cast<StepCoef *>(g.ws + w.step_table);
     int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
     for (int64_t s0 = 0; rc == COLATUS_OK && s0 < n_steps; s0 += RUN_CHUNK) {
@@ -663,7 +732,7 @@ static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t
             if (use_graph) {
                 e = cudaGraphLaunch(g.graph_exec, g.run_stream);
                 if (e != cudaSuccess) rc = fail(COLATUS_CUDA_ERROR, "cudaGraphLaunch failed: %s", cudaGetErrorString(e));
-                g.launches += per_step;
+                g.launches += g.graph_launches;
             } else {
                 rc = enqueue_step_table(g.run_stream);
             }

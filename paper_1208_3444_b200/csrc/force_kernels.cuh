@@ -307,6 +307,30 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
     }
 }
 
+constexpr int REDUCE_MAX_SPLITS = 16;   // upper bound on source splits (partials held in registers below)
+
+// Sum of the `splits` partials of target t in split order 0, 1, 2, ...: all loads first (independent, so
+// their latencies overlap), then the adds in fixed order.
+__device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partial, int64_t stride, int splits,
+                                               int64_t t) {
+    constexpr int MAXS = REDUCE_MAX_SPLITS;
+    float4 q[MAXS];
+#pragma unroll
+    for (int k = 0; k < MAXS; ++k)
+        q[k] = k < splits ? partial[(size_t)k * stride + t] : make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 s = q[0];
+#pragma unroll
+    for (int k = 1; k < MAXS; ++k) {
+        if (k < splits) {
+            s.x += q[k].x;
+            s.y += q[k].y;
+            s.z += q[k].z;
+            s.w += q[k].w;
+        }
+    }
+    return s;
+}
+
 // ---- fixed-order reduction of the source-split partials, applies G ---------------------------------
 template <bool POT>
 __global__ void __launch_bounds__(256) reduce_partials_kernel(const float4 *__restrict__ partial, int64_t stride,
@@ -315,14 +339,7 @@ __global__ void __launch_bounds__(256) reduce_partials_kernel(const float4 *__re
                                                              float4 *__restrict__ out) {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= t_count) return;
-    float4 s = partial[t];
-    for (int k = 1; k < splits; ++k) {
-        const float4 q = partial[(size_t)k * stride + t];
-        s.x += q.x;
-        s.y += q.y;
-        s.z += q.z;
-        s.w += q.w;
-    }
+    const float4 s = sum_partials(partial, stride, splits, t);
     float pot = 0.f;
     if (POT) {
         const float mk = __ldg(pos_mass + t_begin + t).w;

@@ -10,6 +10,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "force_kernels.cuh"
+
 namespace colatus {
 
 // eq. (3): x += d v   (mass in .w untouched)
@@ -104,6 +106,82 @@ kick_drift_table_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel,
     if (TRACE) {
         const int32_t t = trace_slot[begin + i];
         if (t >= 0) ring[(size_t)c.ring_row * trace_k + t] = make_float4(v.x, v.y, v.z, c.tag);
+    }
+}
+
+// ---- fused step kernels (whole-range steps without external terms) ----------------------------------------
+// A leapfrog step is launch-bound at small N, so the two O(N) passes next to the force kernel are folded
+// into their neighbours: drift + staging (eq. (3) and the padded source copy the force kernel reads), and
+// partial-sum reduction + kick + drift (+ tracer record) (eqs. (4), (5)).  Three launches per step instead of
+// five; the arithmetic, statement for statement, is that of drift_kernel / stage_sources_kernel /
+// reduce_partials_kernel / kick_drift_kernel, so the results are bitwise the same.
+// Coefficients come from the scalar arguments, or -- table != nullptr -- from the device table row the step
+// counters select (see the table-driven variants above).
+struct StepSrc {
+    const StepCoef *table;   // nullptr: use the scalars below
+    int *ctr;
+    float d1, cv, ck, d2, tag;
+    int ring_row;
+};
+
+__global__ void __launch_bounds__(256)
+drift_stage_kernel(float4 *__restrict__ pos_mass, const float4 *__restrict__ vel, int64_t n, int64_t n_pad,
+                   float4 *__restrict__ staged, int *__restrict__ mass_flag, int generation, StepSrc src) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float d = src.d1;
+    if (src.table) {
+        const int s = src.ctr[0];
+        if (j == 0) src.ctr[1] = s;
+        d = src.table[s].d1;
+    }
+    if (j >= n_pad) return;
+    if (j < n) {
+        const float m0 = pos_mass[0].w;          // body 0's mass: its .w is never changed by the drift
+        float4 p = pos_mass[j];
+        const float4 v = vel[j];
+        p.x = fmaf(d, v.x, p.x);
+        p.y = fmaf(d, v.y, p.y);
+        p.z = fmaf(d, v.z, p.z);
+        pos_mass[j] = p;
+        staged[j] = p;
+        if (p.w != m0) mass_flag[0] = generation;
+    } else {
+        staged[j] = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+    }
+}
+
+template <bool TRACE>
+__global__ void __launch_bounds__(256)
+reduce_kick_drift_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, float4 *__restrict__ acc,
+                         const float4 *__restrict__ partial, int64_t stride, int splits, int64_t n, float G,
+                         StepSrc src, const int32_t *__restrict__ trace_slot, float4 *__restrict__ ring,
+                         int trace_k) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float cv = src.cv, ck = src.ck, d2 = src.d2, tag = src.tag;
+    int ring_row = src.ring_row;
+    if (src.table) {
+        const int s = src.ctr[1];
+        if (i == 0) src.ctr[0] = s + 1;
+        const StepCoef c = src.table[s];
+        cv = c.cv; ck = c.ck; d2 = c.d2; tag = c.tag; ring_row = c.ring_row;
+    }
+    if (i >= n) return;
+    const float4 s4 = sum_partials(partial, stride, splits, i);
+    const float4 f = make_float4(s4.x * G, s4.y * G, s4.z * G, 0.f);
+    acc[i] = f;                                   // the caller's acc buffer still receives F
+    float4 p = pos_mass[i];
+    float4 v = vel[i];
+    v.x = fmaf(ck, f.x, cv * v.x);
+    v.y = fmaf(ck, f.y, cv * v.y);
+    v.z = fmaf(ck, f.z, cv * v.z);
+    p.x = fmaf(d2, v.x, p.x);
+    p.y = fmaf(d2, v.y, p.y);
+    p.z = fmaf(d2, v.z, p.z);
+    vel[i] = v;
+    pos_mass[i] = p;
+    if (TRACE) {
+        const int32_t t = trace_slot[i];
+        if (t >= 0) ring[(size_t)ring_row * trace_k + t] = make_float4(v.x, v.y, v.z, tag);
     }
 }
 
