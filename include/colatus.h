@@ -138,8 +138,8 @@ int colatus_step_coeffs(double d1, double cv, double ck, double d2);
  * c == NULL means a static background (a = 1, H = 0; a_start ignored).  The per-step
  * coefficients go to a device table (in the workspace, 1024 steps per upload) and a device
  * counter selects the row, so every step launches the same kernels with the same arguments:
- * with use_graph != 0 one captured CUDA graph of the step (drift, stage, force, reduce,
- * kick-drift + tracer record) is replayed per step -- this is what makes the launch-bound
+ * with use_graph != 0 one captured CUDA graph of the step (drift + staging, force, partial-sum
+ * reduction + kick + drift + tracer record) is replayed per step -- this is what makes the launch-bound
  * small-N loops (configs 1-3) fast; with use_graph == 0 the same kernels are launched one by
  * one (for comparison).  Results are bitwise identical to n_steps calls of colatus_step.
  * The loop runs on a stream owned by the library, ordered after everything already enqueued
