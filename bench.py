@@ -168,6 +168,7 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
+    oracle.build()
     from paper_1208_3444_b200 import inputs
     cfg, pm, _ = inputs.make_config(args.config, args.n or None)
     n = pm.shape[0]
@@ -196,6 +197,8 @@ def run_reference(args):
 
 # --------------------------------------------------------------------------------------------------
 def run_native(args):
+    from paper_1208_3444_b200 import build as cuda_build
+    cuda_build.build()                      # no-op when libcolatus.so is up to date (atomic replace otherwise)
     import torch
     import torch.distributed as dist
     from paper_1208_3444_b200 import binding as B
