@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcolatus.so")
 SOURCES = ["colatus_api.cu", "cosmo_host.cpp"]
-HEADERS = ["force_kernels.cuh", "integrate_kernels.cuh", os.path.join("..", "..", "include", "colatus.h")]
+HEADERS = ["force_kernels.cuh", "integrate_kernels.cuh", "analysis_kernels.cuh", "calibrate_kernels.cuh", os.path.join("..", "..", "include", "colatus.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--cudart", "static"]
 
