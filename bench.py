@@ -6,8 +6,8 @@
 Workload (config.workload): BASELINE.json configs[3] -- N = 2^20 bodies, 64 Gaussian clusters +
 50 % uniform background, log-normal masses, eps = 1e-3, synthetic and seeded
 (paper_1208_3444_b200/inputs.py).  One "step" is one pass of the whole hot path (SURVEY 8a rows
-a1-a7): host Friedmann mid-step values (eq. 2), colatus_step = drift (eq. 3) -> repack -> force
-kernel (eq. 1) -> partial reduce -> fused kick-drift + tracer record (eqs. 4-5), then
+a1-a7): host Friedmann mid-step values (eq. 2), colatus_step = drift + source staging (eq. 3) -> force
+kernel (eq. 1) -> partial reduce + kick + drift + tracer record (eqs. 4-5), then
 colatus_diagnostics (momentum / kinetic energy reductions).  N^2 pair interactions per step;
 20 flop per interaction (BASELINE convention).
 

@@ -71,7 +71,7 @@ typedef struct colatus_config {
 /* Cosmological model of eq. (2): H0 and the four density parameters today. */
 typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosmo;
 
-/* Bytes of device workspace needed for problems up to n_max bodies: the repacked
+/* Bytes of device workspace needed for problems up to n_max bodies: the staged (padded)
  * source array, source-split partial sums, reduction scratch, and staging for the
  * host-buffer entry point.  Pure host arithmetic; 0 if n_max < 1. */
 size_t colatus_workspace_bytes(int64_t n_max);

@@ -376,7 +376,7 @@ int enqueue_step_scalar(double d1, double cv, double ck, double d2, float tag) {
 void invalidate_graph() { g.graph_valid = false; }
 
 // One step with the coefficients of table row ctr[0] (integrate_kernels.cuh "table-driven variants"):
-// the same five launches as colatus_step, with step-independent arguments, on stream `st`.
+// the same launches as colatus_step (fused when possible), with step-independent arguments, on stream `st`.
 int enqueue_step_table(cudaStream_t st) {
     const Workspace w = workspace_layout(g.n);
     const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
