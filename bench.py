@@ -53,8 +53,9 @@ def parse():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-step-loops", action="store_true", help="skip the configs 1-3 steps/s side measurement")
-    ap.add_argument("--config", type=int, default=WORKLOAD_CONFIG, choices=[4, 5],
-                    help="4 = N=2^20 (the reported workload, default); 5 = N=2^22 (the at-scale case of BASELINE.json)")
+    ap.add_argument("--config", type=int, default=WORKLOAD_CONFIG, choices=[2, 3, 4, 5],
+                    help="4 = N=2^20 (the reported workload, default); 5 = N=2^22 (the at-scale case of BASELINE.json); "
+                         "2, 3 = the equal-mass stepping configurations (N = 32768, 131072), for profiling the equal-mass loop")
     ap.add_argument("--n", type=int, default=0, help="override N (debug only; the reported workload is 2^20)")
     return ap.parse_args()
 
@@ -327,8 +328,12 @@ def run_native(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"config {cfg.index}: N={n}, {64 if cfg.index == 4 else 256} Gaussian clusters + 50% uniform background, "
-                                   f"log-normal masses, eps={cfg.eps}; one full leapfrog step + diagnostics per step",
+            "config": {"workload": f"config {cfg.index} ({cfg.name}): N={n}, " +
+                                   ({4: "64 Gaussian clusters + 50% uniform background, log-normal masses",
+                                     5: "256 Gaussian clusters + 50% uniform background, log-normal masses",
+                                     3: "Plummer sphere + 30% uniform background, equal masses",
+                                     2: "32^3 lattice + Gaussian displacements, equal masses"}[cfg.index]) +
+                                   f", eps={cfg.eps}; one full leapfrog step + diagnostics per step",
                        "n": n, "interactions_per_step": float(n) * n, "tracers": N_TRACERS,
                        "parallelism": "single GPU" if world == 1 else f"targets sharded over {world} GPUs, "
                                                                        "all-gather of positions per drift",
