@@ -230,3 +230,31 @@ def test_all_zero_and_nan_masses(session):
     q[0, 3] = np.nan                                     # NaN in body 0: every comparison is unequal
     out = session.forces(q, cfg.eps2).cpu().numpy()
     assert np.isnan(out[1:, :3]).all()
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_forces_random_scales_offsets_and_mass_ranges(session, seed):
+    """Seeded random problems far from the unit box: sizes 2..6000, box scales 1e-3..1e3, offsets up to 50 box
+    lengths (differences of nearby FP32 coordinates are exact, so the tolerances must still hold), softening
+    from 1e-3 to 0.3 of the box, masses over six decades, uniform / clustered / planar layouts."""
+    rng = np.random.Generator(np.random.PCG64(7000 + seed))
+    n = int(rng.integers(2, 6000))
+    scale = 10.0 ** rng.uniform(-3, 3)
+    offset = scale * rng.uniform(-50, 50, size=3)
+    layout = seed % 3
+    if layout == 0:
+        x = rng.random((n, 3))
+    elif layout == 1:
+        centres = rng.random((5, 3))
+        x = centres[rng.integers(0, 5, n)] + 0.01 * rng.standard_normal((n, 3))
+    else:
+        x = rng.random((n, 3)) * np.array([1.0, 1.0, 1e-3])           # a thin sheet
+    pm = np.empty((n, 4), dtype=np.float32)
+    pm[:, :3] = (offset + scale * x).astype(np.float32)
+    pm[:, 3] = (10.0 ** rng.uniform(-6, 0, n)).astype(np.float32)
+    eps2 = np.float32((scale * 10.0 ** rng.uniform(-3, -0.5)) ** 2)
+    out = session.forces(pm, eps2, potential=True).cpu().numpy()
+    ref, phi = oracle.forces(pm, eps2, 1.0, potential=True)
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (seed, n, scale, med, mx)
+    assert np.allclose(out[:, 3], phi, rtol=5e-5, atol=0)
