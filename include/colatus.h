@@ -35,6 +35,11 @@
  *   - Device data are not scanned: NaN/Inf inputs give NaN outputs, not errors.
  *   - Results are bit-reproducible run to run for a fixed (n, device, build):
  *     no floating-point atomics anywhere.
+ *   - Equal masses are detected on the device at every force evaluation (all m_j equal to
+ *     m_0 in value): the kernel then applies the common mass once to the finished sums instead
+ *     of once per pair (one rounding fewer per term).  No flag, no host round trip; a NaN or a
+ *     single different mass selects the general loop.  Positions must stay well below 1e18 in
+ *     magnitude (padding bodies of mass 0 sit there).
  */
 #ifndef COLATUS_H
 #define COLATUS_H
