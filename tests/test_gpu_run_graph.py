@@ -34,7 +34,7 @@ def _run(cfg, pm, vel, steps, mode, tracers=None, capacity=None):
     return a_end, pos, v, diag, ring
 
 
-@pytest.mark.parametrize("index,n_override,steps", [(1, None, 12), (2, 4913, 7), (3, 9001, 6)])
+@pytest.mark.parametrize("index,n_override,steps", [(1, None, 12), (2, 4913, 7), (3, 9001, 6), (3, 100, 9), (1, 2, 5)])
 def test_run_equals_step_loop_bitwise(index, n_override, steps):
     cfg, pm, vel = inputs.make_config(index, n_override)
     rng = np.random.Generator(np.random.PCG64(9))

@@ -176,3 +176,32 @@ def test_target_range_stepping_matches_full():
         pos[:h] = new_pos[0].cpu().numpy()
         pos[h:] = new_pos[1].cpu().numpy()
     assert np.allclose(pos, full_pos, rtol=0, atol=1e-7) and np.allclose(v, full_vel, rtol=2e-6, atol=1e-7)
+
+
+@pytest.mark.parametrize("index,n_override", [(1, None), (3, 100), (3, 20000)])
+def test_fused_step_equals_separate_kernels_bitwise(index, n_override):
+    """colatus_step_coeffs takes the fused route (drift+staging, force, reduce+kick+drift); colatus_drift +
+    colatus_force_kick_drift take the separate kernels.  Same arithmetic, statement for statement: positions,
+    velocities, the acc buffer and the tracer ring must agree to the bit (single- and multi-split sizes)."""
+    cfg, pm, vel = inputs.make_config(index, n_override)
+    rng = np.random.Generator(np.random.PCG64(3))
+    vel = vel.copy()
+    vel[:, :3] = 0.02 * rng.standard_normal((cfg.n, 3)).astype(np.float32)
+    tr = np.arange(0, cfg.n, max(cfg.n // 8, 1), dtype=np.int32)[:8]
+    coeffs = [(0.4e-3, 0.9, 1.1e-3, 0.6e-3), (0.5e-3, 1.0, 0.7e-3, 0.5e-3), (0.3e-3, 0.8, 2.0e-3, 0.2e-3)]
+    outs = []
+    for fused in (True, False):
+        with _session(cfg.G, cfg.n) as s:
+            s.upload(pm, vel, cfg.eps2)
+            s.trace(tr, 2)
+            for d1, cv, ck, d2 in coeffs:
+                if fused:
+                    B.colatus_step_coeffs(d1, cv, ck, d2)
+                else:
+                    B.colatus_drift(d1)
+                    B.colatus_force_kick_drift(cv, ck, d2)
+            pos, v = s.download()
+            outs.append((pos, v, s.acc.cpu().numpy(), s.ring.cpu().numpy(), s.diagnostics(1.0)[12]))
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b)
+    assert outs[0][4] == len(coeffs)
