@@ -271,6 +271,13 @@ int64_t  colatus_launch_count(void);
  * duration.  Runs on the default stream and synchronises. */
 int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out);
 
+/* Issue-rule probes behind DESIGN.md 6.2: register-only loops of 12 packed FP32 ops per group plus
+ * mode 0: nothing; 1: 2 MUFU.RSQ; 2: 2 integer adds; 3: the 12 ops with three distinct 64-bit register
+ * operands each; 4: one broadcast LDS.128; 5: 24 scalar FFMA + 2 MUFU.RSQ instead.  *cycles_per_group =
+ * SMSP cycles one group costs (launch time x max SM clock / groups per SMSP; 24 = FMA pipe saturated).
+ * Default stream, synchronises. */
+int colatus_pipe_probe(int mode, double *cycles_per_group);
+
 /* Geometry the force path picked for n bodies / target_count targets on this device:
  * out[0] = targets per CTA, out[1] = target tiles, out[2] = source splits,
  * out[3] = sources per split (padded), out[4] = CTAs per SM, out[5] = SM count,

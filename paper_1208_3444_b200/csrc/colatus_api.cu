@@ -968,6 +968,43 @@ int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out) {
     return COLATUS_OK;
 }
 
+int colatus_pipe_probe(int mode, double *cycles_per_group) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!cycles_per_group || mode < 0 || mode > 5) return fail(COLATUS_INVALID_ARG, "mode must be 0..5, output non-null");
+    float *sink = reinterpret_cast<float *>(g.ws + 128);
+    const int blocks = g.sm_count * 8 * 8;                      // 8 full waves of 8 CTAs/SM (16 warps per SMSP)
+    int clock_khz = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&clock_khz, cudaDevAttrClockRate, g.device));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    float best = 0.f;
+    cudaError_t err = cudaSuccess;
+    for (int r = 0; r < 4 && err == cudaSuccess; ++r) {
+        cudaEventRecord(e0, nullptr);
+        switch (mode) {
+            case 0: pipe_probe_kernel<0><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
+            case 1: pipe_probe_kernel<1><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
+            case 2: pipe_probe_kernel<2><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
+            case 3: pipe_probe_kernel<3><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
+            case 4: pipe_probe_kernel<4><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
+            default: pipe_probe_kernel<5><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
+        }
+        cudaEventRecord(e1, nullptr);
+        err = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && (best == 0.f || ms < best)) best = ms;
+        g.launches++;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (err != cudaSuccess) return fail(COLATUS_CUDA_ERROR, "probe failed: %s", cudaGetErrorString(err));
+    const double groups_per_smsp = (double)blocks * (CAL_THREADS / 32) * PROBE_GROUPS / ((double)g.sm_count * 4.0);
+    *cycles_per_group = (double)best * 1e-3 * (double)clock_khz * 1e3 / groups_per_smsp;   // at the max SM clock
+    return COLATUS_OK;
+}
+
 int64_t colatus_launch_count(void) { return g.launches; }
 
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]) {
