@@ -14,8 +14,10 @@ colatus_diagnostics (momentum / kinetic energy reductions).  N^2 pair interactio
 --impl reference times the FP64 CPU oracle (oracle/) on the host cores on a bounded sample of the
 same workload; it is a deliberately slow baseline, not the target.
 
-N > 1 (torchrun, one rank per GPU): eq. (1) sharded by targets, positions all-gathered over NCCL
-after each drift (the path's only exchange step); total work fixed -> "scaling": "strong".
+N > 1 (one rank per GPU): eq. (1) sharded by targets, positions all-gathered over NCCL once per step after
+the first drift (the path's only exchange step), diagnostics by one all-reduce; total work fixed ->
+"scaling": "strong".  Under torchrun the ranks come from the environment; a plain `python bench.py --gpus N`
+re-launches itself under torch.distributed.run with N ranks (and fails loudly if fewer GPUs are visible).
 """
 from __future__ import annotations
 
@@ -36,9 +38,14 @@ WORKLOAD_CONFIG = 4                        # BASELINE.json configs[3]: N = 2^20
 FLOP_PER_INTERACTION = 20.0                # BASELINE.json convention
 SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
-# dram__bytes_read.sum + dram__bytes_write.sum of one force-kernel launch at N = 2^20 from the
-# `ncu --set full` capture summarised in profiles/ (None until that capture exists).
-FORCE_KERNEL_DRAM_TRAFFIC_BYTES = 130877184     # profiles/r01_force_kernel_ncu_full.txt
+# dram__bytes_read.sum + dram__bytes_write.sum of one force-kernel launch from the `ncu --set full` capture
+# summarised in profiles/: valid only for the (n, source splits) it was captured at -- reported as null otherwise.
+FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 130877184, "n": 1 << 20, "splits": 8,
+                             "profile": "profiles/r01_force_kernel_ncu_full.txt"}
+# executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
+# (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention
+EXECUTED_FLOP_GENERAL, EXECUTED_FLOP_EQUAL_MASS = 19.0, 18.0
+FMA_PIPE_LANE_OPS_GENERAL, FMA_PIPE_LANE_OPS_EQUAL_MASS = 12.0, 11.0
 METRIC = "Ginteractions/s softened direct-sum gravity at N=2^20; % of FP32 FMA peak"
 UNIT = "Ginteractions/s"
 BENCH_TAU = 1.0e-6                         # step size of the bench steps (EdS background from a = 0.02)
@@ -53,6 +60,7 @@ def parse():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-step-loops", action="store_true", help="skip the configs 1-3 steps/s side measurement")
+    ap.add_argument("--no-config5", action="store_true", help="skip the N = 2^22 side leg (1 warm-up + 2 timed steps)")
     ap.add_argument("--config", type=int, default=WORKLOAD_CONFIG, choices=[2, 3, 4, 5],
                     help="4 = N=2^20 (the reported workload, default); 5 = N=2^22 (the at-scale case of BASELINE.json); "
                          "2, 3 = the equal-mass stepping configurations (N = 32768, 131072), for profiling the equal-mass loop")
@@ -197,9 +205,31 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------------
-def run_native(args):
-    from paper_1208_3444_b200 import build as cuda_build
-    cuda_build.build()                      # no-op when libcolatus.so is up to date (atomic replace otherwise)
+WORKLOAD_TEXT = {4: "64 Gaussian clusters + 50% uniform background, log-normal masses",
+                 5: "256 Gaussian clusters + 50% uniform background, log-normal masses",
+                 3: "Plummer sphere + 30% uniform background, equal masses",
+                 2: "32^3 lattice + Gaussian displacements, equal masses"}
+
+
+def relaunch_with_ranks(args):
+    """`python bench.py --gpus N` without torchrun: start N ranks (one per GPU) of this same command under
+    torch.distributed.run on 127.0.0.1 and replace this process with it.  Fails loudly if the box has fewer GPUs."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible; refusing to run fewer "
+                         "ranks than requested (the sharded path needs one GPU per rank)")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
+def measure(args, config_index, n_override, steps, warmup, world, rank, local_rank, with_e2e):
+    """W warm-up + K timed passes of the whole hot path on one configuration; returns the pieces of the JSON line."""
     import torch
     import torch.distributed as dist
     from paper_1208_3444_b200 import binding as B
@@ -207,42 +237,31 @@ def run_native(args):
     from paper_1208_3444_b200.harness import Session
     from paper_1208_3444_b200.sharded import LibcolatusOps, ShardedStepper, partition
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py --impl native needs a CUDA device (libcolatus has no CPU fallback)")
-    torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    cfg, pm, vel = inputs.make_config(args.config, args.n or None)
+    cfg, pm, vel = inputs.make_config(config_index, n_override)
     n = pm.shape[0]
     cosmo = inputs.Cosmology(H0=float(np.sqrt(8.0 * np.pi / 3.0)), Om_M=1.0)     # EdS, as config 1
     sess = Session(cfg.G, n, device=local_rank)
     begin, count = partition(n, world, rank)
     sess.upload(pm, vel, cfg.eps2)
+    tr_idx = (np.arange(N_TRACERS, dtype=np.int64) * (n // N_TRACERS)).astype(np.int32)
+    stepper = None
     if world > 1:
         sess.acc = torch.zeros((count, 4), dtype=torch.float32, device=sess.device)
         ops = LibcolatusOps(sess.pos, sess.vel, sess.acc, n, cfg.eps2, begin, count)
         stepper = ShardedStepper(sess.pos, n, ops)
-    tr_idx = (np.arange(N_TRACERS, dtype=np.int64) * (n // N_TRACERS)).astype(np.int32)
-    sess.trace(tr_idx, max(args.steps + args.warmup, 1))
+    sess.trace(tr_idx, max(steps + warmup, 1))
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=sess.device)       # > 126 MB L2
-
     state = {"a": 0.02}
-    # measured denominator (register-only FMA loops through the C ABI), beside the derived 74.45 TFLOP/s
-    cal_ffma, _ = B.colatus_calibrate_fp32(0)
-    cal_ffma2, _ = B.colatus_calibrate_fp32(1)
 
     def one_step():
         a_mid = B.colatus_a_advance(cosmo, state["a"], 0.5 * BENCH_TAU)              # a1 (host, double)
         H_mid = B.colatus_hubble(cosmo, a_mid)
-        if world > 1:
-            stepper.step(BENCH_TAU, a_mid, H_mid)                                    # a2-a6, sharded
+        if stepper is not None:
+            stepper.step(BENCH_TAU, a_mid, H_mid)                                    # a2-a6, sharded; 1 all-gather
+            d = stepper.diagnostics(a_mid, False)                                    # a7: 1 all-reduce (syncs)
         else:
             B.colatus_step(BENCH_TAU, a_mid, H_mid)                                  # a2-a6
-        d = B.colatus_diagnostics(a_mid, False)                                      # a7 (syncs)
+            d = B.colatus_diagnostics(a_mid, False)                                  # a7 (syncs)
         state["a"] = B.colatus_a_advance(cosmo, a_mid, 0.5 * BENCH_TAU)
         flush_buf.zero_()                                                            # L2 flush between steps
         return d
@@ -252,7 +271,7 @@ def run_native(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         one_step()
     barrier()
     B.colatus_profile(True)
@@ -262,7 +281,7 @@ def run_native(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         diag = one_step()
     e1.record()
     barrier()
@@ -275,76 +294,131 @@ def run_native(args):
         t = torch.tensor([ms_total], dtype=torch.float64, device=sess.device)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
-    ms_step = ms_total / args.steps
+    ms_step = ms_total / steps
     value = float(n) * n / (ms_step * 1e-3) / 1e9
 
     # ---- roofline of the dominant kernel (force kernel), from events inside the timed region
     pairs_per_launch = float(count) * n
     geo = B.colatus_force_geometry(n, count)
+    equal_mass = bool(np.all(pm[:, 3] == pm[0, 3]))
     k_ms = kernel_ms / max(kernel_launches, 1)
-    achieved = FLOP_PER_INTERACTION * pairs_per_launch / (k_ms * 1e-3) / 1e12
+    per_s = pairs_per_launch / (k_ms * 1e-3)
+    achieved = FLOP_PER_INTERACTION * per_s / 1e12
+    cap = FORCE_KERNEL_DRAM_TRAFFIC
+    traffic = cap["bytes"] if (n == cap["n"] and world == 1 and geo["source_splits"] == cap["splits"]) else None
+    lane_ops = FMA_PIPE_LANE_OPS_EQUAL_MASS if equal_mass else FMA_PIPE_LANE_OPS_GENERAL
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / FP32_PEAK_TFLOPS, "traffic": FORCE_KERNEL_DRAM_TRAFFIC_BYTES if (n == 1 << 20 and world == 1) else None,
-                "kernel": "force_kernel<%d,%d,4,false,2>" % (geo["targets_per_thread"] // 2,
-                                                             {6: 512, 4: 512, 2: 256}[geo["targets_per_thread"]]),
+                "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+                "traffic_from": cap["profile"] if traffic else None,
+                "algorithmic_bytes": 16 * n * (2 + (geo["source_splits"] if geo["source_splits"] > 1 else 0)),
+                "kernel": "force_kernel<%d,%d,4,false,2>%s" % (geo["targets_per_thread"] // 2,
+                                                                 {6: 512, 4: 512, 2: 256}[geo["targets_per_thread"]],
+                                                                 " equal-mass loop" if equal_mass else ""),
                 "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / ms_step,
                 "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); "
                               "no FP32 figure in MEASURED_PEAKS.json",
-                "peak_measured": {"ffma_tflops": cal_ffma, "ffma2_tflops": cal_ffma2,
-                                  "how": "colatus_calibrate_fp32: register-only FFMA / FFMA2 loops, best of 3"},
-                "frac_of_measured_peak": achieved / max(cal_ffma, cal_ffma2),
                 "flop_per_interaction": FLOP_PER_INTERACTION,
+                "frac_executed_flops": (EXECUTED_FLOP_EQUAL_MASS if equal_mass else EXECUTED_FLOP_GENERAL) * per_s
+                                       / 1e12 / FP32_PEAK_TFLOPS,
+                "fma_pipe_busy_frac": lane_ops * per_s / (SM_COUNT * FP32_LANES * SM_MAX_MHZ * 1e6),
                 "frac_at_sampled_clock": (achieved / (FP32_PEAK_TFLOPS * clocks["sm_mhz"] / SM_MAX_MHZ)
                                           if clocks.get("sm_mhz") else None)}
 
     # ---- end to end through the C ABI with HOST buffers (N = 1 only: the call is single-GPU)
     e2e = None
-    if world == 1:
+    if world == 1 and with_e2e:
         h_in = torch.from_numpy(pm).pin_memory()
         h_out = torch.empty((n, 4), dtype=torch.float32).pin_memory()
         B.colatus_forces_host(h_in, n, cfg.eps2, h_out)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             B.colatus_forces_host(h_in, n, cfg.eps2, h_out)          # H2D + eq. (1) + D2H + sync
         dt = time.perf_counter() - t0
-        e2e = {"value": args.steps * float(n) * n / dt / 1e9, "unit": UNIT,
+        e2e = {"value": steps * float(n) * n / dt / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
-               "call": "colatus_forces_host (pinned host buffers)", "ms_per_step": dt / args.steps * 1e3}
+               "call": "colatus_forces_host (pinned host buffers)", "ms_per_step": dt / steps * 1e3}
+    sess.close()
+    return {"cfg": cfg, "pm": pm, "n": n, "value": value, "ms_step": ms_step, "roofline": roofline, "e2e": e2e,
+            "launches": int(launches), "clocks": clocks, "geo": geo, "diag": diag}
+
+
+def run_native(args):
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.gpus > 1 and world_env is None:
+        relaunch_with_ranks(args)                # does not return
+    from paper_1208_3444_b200 import build as cuda_build
+    cuda_build.build()                      # no-op when the libraries are up to date (atomic replace otherwise)
+    import torch
+    import torch.distributed as dist
+    from paper_1208_3444_b200 import probe as P
+
+    world = int(world_env or "1")
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch one rank per GPU")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl native needs a CUDA device (libcolatus has no CPU fallback)")
+    if torch.cuda.device_count() <= local_rank:
+        raise SystemExit(f"bench.py: rank {rank} has no GPU (LOCAL_RANK={local_rank}, "
+                         f"{torch.cuda.device_count()} visible)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    # measured denominator (register-only FMA loops of libcolatus_probe), beside the derived 74.45 TFLOP/s
+    cal_ffma, _ = P.fp32_peak(False, local_rank)
+    cal_ffma2, _ = P.fp32_peak(True, local_rank)
+
+    m = measure(args, args.config, args.n or None, args.steps, args.warmup, world, rank, local_rank, True)
+    cfg, pm, n = m["cfg"], m["pm"], m["n"]
+    roofline = m["roofline"]
+    roofline["peak_measured"] = {"ffma_tflops": cal_ffma, "ffma2_tflops": cal_ffma2,
+                                 "how": "libcolatus_probe: register-only FFMA / FFMA2 loops, best of 3"}
+    roofline["frac_of_measured_peak"] = roofline["achieved"] / max(cal_ffma, cal_ffma2)
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, cores, sample = oracle_sample_rate(pm, cfg)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
-    sess.close()
+    default_run = world == 1 and not args.n and args.config == WORKLOAD_CONFIG
     step_loops = None
-    if rank == 0 and world == 1 and not args.no_step_loops and not args.n and args.config == WORKLOAD_CONFIG:
+    if rank == 0 and default_run and not args.no_step_loops:
         step_loops = step_loop_rates(local_rank)
 
+    # side leg: the at-scale case of BASELINE.json (configs[4], N = 2^22): 1 warm-up + 2 timed steps
+    config5 = None
+    if rank == 0 and default_run and not args.no_config5:
+        del pm
+        m5 = measure(args, 5, None, 2, 1, 1, 0, local_rank, False)
+        config5 = {"n": m5["n"], "steps": 2, "warmup": 1, "ms_per_step": m5["ms_step"], "value": m5["value"],
+                   "unit": UNIT, "frac": m5["roofline"]["frac"], "kernel_ms": m5["roofline"]["kernel_ms"],
+                   "kernel": m5["roofline"]["kernel"], "geometry": m5["geo"],
+                   "clocks": m5["clocks"]}
+
     if rank == 0:
+        value = m["value"]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "warmup": args.warmup, "ms_per_step": m["ms_step"], "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"config {cfg.index} ({cfg.name}): N={n}, " +
-                                   ({4: "64 Gaussian clusters + 50% uniform background, log-normal masses",
-                                     5: "256 Gaussian clusters + 50% uniform background, log-normal masses",
-                                     3: "Plummer sphere + 30% uniform background, equal masses",
-                                     2: "32^3 lattice + Gaussian displacements, equal masses"}[cfg.index]) +
+            "config": {"workload": f"config {cfg.index} ({cfg.name}): N={n}, " + WORKLOAD_TEXT[cfg.index] +
                                    f", eps={cfg.eps}; one full leapfrog step + diagnostics per step",
                        "n": n, "interactions_per_step": float(n) * n, "tracers": N_TRACERS,
                        "parallelism": "single GPU" if world == 1 else f"targets sharded over {world} GPUs, "
-                                                                       "all-gather of positions per drift",
+                                                                       "one all-gather of positions per step, "
+                                                                       "one all-reduce of 16 doubles for the diagnostics",
                        "l2_flush": "256 MiB memset between steps (inside the timed region)",
-                       "geometry": geo},
+                       "geometry": m["geo"]},
             "gflops": value * FLOP_PER_INTERACTION,
             "frac_fp32_peak": value * FLOP_PER_INTERACTION / 1e3 / (FP32_PEAK_TFLOPS * world),
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
-            "gpu_launches": int(launches), "clocks": clocks,
-            "step_loops": step_loops,
-            "diagnostics_last_step": {"M": diag[0], "T": diag[7]},
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": m["e2e"],
+            "gpu_launches": m["launches"], "clocks": m["clocks"],
+            "step_loops": step_loops, "config5": config5,
+            "diagnostics_last_step": {"M": float(m["diag"][0]), "T": float(m["diag"][7])},
             "paper_context": "paper reports no timing; largest run 32^3 particles on a GTX680 (PAPER.md:23)",
         }
         print(json.dumps(line), flush=True)

@@ -89,7 +89,10 @@ void colatus_shutdown(void);
 /* ---- eq. (1): stateless force evaluation on caller-owned device arrays -------------
  * pos_mass_dev : const float4[n]  (x, y, z, m)
  * acc_out_dev  : float4[n]        (F_x, F_y, F_z, 0)  with G applied, a^-3 NOT applied
- * eps2         : eps^2 (the paper's min_dist^2), finite, >= 1e-30
+ * eps2         : eps^2 (the paper's min_dist^2), finite, >= 1e-24.  The j = k term is not
+ *                branched around (reading G4): it is m_k eps2^-1.5 * 0 = 0 exactly, PROVIDED m_k eps2^-1.5 is
+ *                finite in FP32 -- the caller keeps |m| * eps2^-1.5 < 3e38 (at the floor: |m| < 3e2), else
+ *                that target's force is NaN.  The same bound keeps close distinct pairs finite.
  * Enqueues on cuda_stream and returns without synchronising.  n in [1, 2^31-1];
  * pointers 16-byte aligned and distinct. */
 int colatus_forces(const void *pos_mass_dev, int64_t n, float eps2, void *acc_out_dev,
@@ -256,6 +259,8 @@ int colatus_diagnostics(double a, int with_potential, double out[16]);
 int colatus_download(float *pos_mass_host, float *vel_host);
 
 /* ---- instrumentation ------------------------------------------------------------------
+ * (Device microbenchmarks -- FP32 peak calibration, issue-rule probes -- are NOT here: they live in the
+ * separate libcolatus_probe, include/colatus_probe.h.)
  * colatus_profile(1) makes the library bracket every force-kernel launch with CUDA events
  * on the launching stream; colatus_profile_read synchronises and returns the number of
  * bracketed launches and their summed duration in ms, then resets both.
@@ -263,20 +268,6 @@ int colatus_download(float *pos_mass_host, float *vel_host);
 int      colatus_profile(int enable);
 int      colatus_profile_read(double *total_ms, int64_t *launches);
 int64_t  colatus_launch_count(void);
-
-/* Measures the plain FP32 FMA throughput of the device with a register-only loop (packed = 0: scalar
- * FFMA; 1: FFMA2 / fma.rn.f32x2): the denominator of the "alu" roofline, which
- * MEASURED_PEAKS.json does not carry.  *tflops = 2 flop x lane-FMAs / best of three timed launches
- * (16 waves of 8 CTAs/SM, 8 independent chains per thread); *ms_out (may be NULL) = that launch's
- * duration.  Runs on the default stream and synchronises. */
-int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out);
-
-/* Issue-rule probes behind DESIGN.md 6.2: register-only loops of 12 packed FP32 ops per group plus
- * mode 0: nothing; 1: 2 MUFU.RSQ; 2: 2 integer adds; 3: the 12 ops with three distinct 64-bit register
- * operands each; 4: one broadcast LDS.128; 5: 24 scalar FFMA + 2 MUFU.RSQ instead.  *cycles_per_group =
- * SMSP cycles one group costs (launch time x max SM clock / groups per SMSP; 24 = FMA pipe saturated).
- * Default stream, synchronises. */
-int colatus_pipe_probe(int mode, double *cycles_per_group);
 
 /* Geometry the force path picked for n bodies / target_count targets on this device:
  * out[0] = targets per CTA, out[1] = target tiles, out[2] = source splits,

@@ -69,8 +69,6 @@ SIGNATURES = {
     "colatus_download": (c_int, [c_void_p, c_void_p]),
     "colatus_profile": (c_int, [c_int]),
     "colatus_profile_read": (c_int, [POINTER(c_double), POINTER(c_int64)]),
-    "colatus_calibrate_fp32": (c_int, [c_int, POINTER(c_double), POINTER(c_double)]),
-    "colatus_pipe_probe": (c_int, [c_int, POINTER(c_double)]),
     "colatus_launch_count": (c_int64, []),
     "colatus_force_geometry": (c_int, [c_int64, c_int64, POINTER(c_int64)]),
     "colatus_set_option": (c_int, [c_char_p, c_int64]),
@@ -291,20 +289,6 @@ def colatus_profile_read():
     ms, k = c_double(0.0), c_int64(0)
     _check(lib().colatus_profile_read(ctypes.byref(ms), ctypes.byref(k)))
     return ms.value, k.value
-
-
-def colatus_calibrate_fp32(packed):
-    """Measured FP32 FMA throughput (TFLOP/s, ms) of a register-only FFMA (packed=0) / FFMA2 (packed=1) loop."""
-    t, ms = c_double(0.0), c_double(0.0)
-    _check(lib().colatus_calibrate_fp32(int(bool(packed)), ctypes.byref(t), ctypes.byref(ms)))
-    return t.value, ms.value
-
-
-def colatus_pipe_probe(mode):
-    """SMSP cycles per group of 12 packed FP32 ops (+ the extras of `mode`, see colatus.h) at the max SM clock."""
-    c = c_double(0.0)
-    _check(lib().colatus_pipe_probe(int(mode), ctypes.byref(c)))
-    return c.value
 
 
 def colatus_launch_count():

@@ -15,7 +15,6 @@
 #include "force_kernels.cuh"
 #include "integrate_kernels.cuh"
 #include "analysis_kernels.cuh"
-#include "calibrate_kernels.cuh"
 
 namespace {
 
@@ -276,6 +275,10 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     return COLATUS_OK;
 }
 
+// The branch-free self term (reading G4) is exactly 0 only while w = m_k rinv^3 stays finite in FP32 (0 * inf = NaN):
+// rinv^3 = eps2^-1.5 <= 1e36 at this floor, which leaves masses up to ~3e2 in magnitude (colatus.h "eps2").
+inline bool eps2_ok(float eps2) { return std::isfinite(eps2) && eps2 >= 1e-24f; }
+
 int check_forces_args(const void *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2,
                       const void *acc_out) {
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
@@ -286,7 +289,7 @@ int check_forces_args(const void *pos_mass, int64_t n, int64_t t_begin, int64_t 
                     (long long)t_count, (long long)n);
     if (!aligned16(pos_mass) || !aligned16(acc_out)) return fail(COLATUS_INVALID_ARG, "pointer not 16-byte aligned");
     if (pos_mass == acc_out) return fail(COLATUS_INVALID_ARG, "pos_mass and acc_out alias");
-    if (!std::isfinite(eps2) || eps2 < 1e-30f) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-30");
+    if (!eps2_ok(eps2)) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-24");
     return COLATUS_OK;
 }
 
@@ -508,7 +511,7 @@ int colatus_forces_host(const float *pos_mass_host, int64_t n, float eps2, float
     if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
     if (!pos_mass_host || !acc_out_host) return fail(COLATUS_INVALID_ARG, "null pointer");
     if (n < 1 || n > 2147483647LL) return fail(COLATUS_INVALID_ARG, "n=%lld out of [1, 2^31-1]", (long long)n);
-    if (!std::isfinite(eps2) || eps2 < 1e-30f) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-30");
+    if (!eps2_ok(eps2)) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-24");
     const Workspace w = workspace_layout(n);
     if (w.total > g.ws_bytes)
         return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
@@ -932,76 +935,6 @@ int colatus_profile_read(double *total_ms, int64_t *launches) {
     *total_ms = sum;
     *launches = (int64_t)(g.ev_used / 2);
     g.ev_used = 0;
-    return COLATUS_OK;
-}
-
-int colatus_calibrate_fp32(int packed, double *tflops, double *ms_out) {
-    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
-    if (!tflops) return fail(COLATUS_INVALID_ARG, "tflops is null");
-    if (workspace_layout(1).total > g.ws_bytes) return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace too small");
-    float *sink = reinterpret_cast<float *>(g.ws + 128);      // never written (see calibrate_kernels.cuh)
-    const int blocks = g.sm_count * 8 * 16;                    // 16 full waves of 8 CTAs/SM
-    cudaEvent_t e0, e1;
-    CUDA_TRY(cudaEventCreate(&e0));
-    CUDA_TRY(cudaEventCreate(&e1));
-    float best = 0.f;
-    cudaError_t err = cudaSuccess;
-    for (int r = 0; r < 4 && err == cudaSuccess; ++r) {        // first repetition is the warm-up
-        cudaEventRecord(e0, nullptr);
-        if (packed)
-            calibrate_fma_kernel<1><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink);
-        else
-            calibrate_fma_kernel<0><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink);
-        cudaEventRecord(e1, nullptr);
-        err = cudaEventSynchronize(e1);
-        float ms = 0.f;
-        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
-        if (r > 0 && (best == 0.f || ms < best)) best = ms;
-        g.launches++;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (err != cudaSuccess) return fail(COLATUS_CUDA_ERROR, "calibration failed: %s", cudaGetErrorString(err));
-    const double lane_fma = (double)blocks * CAL_THREADS * (double)CAL_ITERS * CAL_CHAINS * 2.0;   // per launch
-    *tflops = 2.0 * lane_fma / ((double)best * 1e-3) / 1e12;
-    if (ms_out) *ms_out = best;
-    return COLATUS_OK;
-}
-
-int colatus_pipe_probe(int mode, double *cycles_per_group) {
-    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
-    if (!cycles_per_group || mode < 0 || mode > 5) return fail(COLATUS_INVALID_ARG, "mode must be 0..5, output non-null");
-    float *sink = reinterpret_cast<float *>(g.ws + 128);
-    const int blocks = g.sm_count * 8 * 8;                      // 8 full waves of 8 CTAs/SM (16 warps per SMSP)
-    int clock_khz = 0;
-    CUDA_TRY(cudaDeviceGetAttribute(&clock_khz, cudaDevAttrClockRate, g.device));
-    cudaEvent_t e0, e1;
-    CUDA_TRY(cudaEventCreate(&e0));
-    CUDA_TRY(cudaEventCreate(&e1));
-    float best = 0.f;
-    cudaError_t err = cudaSuccess;
-    for (int r = 0; r < 4 && err == cudaSuccess; ++r) {
-        cudaEventRecord(e0, nullptr);
-        switch (mode) {
-            case 0: pipe_probe_kernel<0><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
-            case 1: pipe_probe_kernel<1><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
-            case 2: pipe_probe_kernel<2><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
-            case 3: pipe_probe_kernel<3><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
-            case 4: pipe_probe_kernel<4><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
-            default: pipe_probe_kernel<5><<<blocks, CAL_THREADS>>>(0.999f, 0.001f, sink); break;
-        }
-        cudaEventRecord(e1, nullptr);
-        err = cudaEventSynchronize(e1);
-        float ms = 0.f;
-        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
-        if (r > 0 && (best == 0.f || ms < best)) best = ms;
-        g.launches++;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (err != cudaSuccess) return fail(COLATUS_CUDA_ERROR, "probe failed: %s", cudaGetErrorString(err));
-    const double groups_per_smsp = (double)blocks * (CAL_THREADS / 32) * PROBE_GROUPS / ((double)g.sm_count * 4.0);
-    *cycles_per_group = (double)best * 1e-3 * (double)clock_khz * 1e3 / groups_per_smsp;   // at the max SM clock
     return COLATUS_OK;
 }
 

@@ -28,6 +28,9 @@ struct Deriv {
 };
 
 // Dormand-Prince 5(4) with step-size control on both components; integrates over `dt` (either sign).
+// If the interval cannot be completed (step size underflows, e.g. a reaches 0 when integrating backwards, or
+// the step guard is exhausted) both components are set to NaN: callers fail loudly instead of using a
+// partial result.
 void dopri(const Deriv &F, double y[2], double dt) {
     static const double c2 = 1.0 / 5, c3 = 3.0 / 10, c4 = 4.0 / 5, c5 = 8.0 / 9;
     static const double a21 = 1.0 / 5;
@@ -78,6 +81,7 @@ void dopri(const Deriv &F, double y[2], double dt) {
         h *= std::fmin(5.0, std::fmax(0.1, fac));
         if (std::fabs(h) < 1e-300) break;
     }
+    if ((dt - t) * dir > 0) y[0] = y[1] = std::numeric_limits<double>::quiet_NaN();
 }
 
 }  // namespace

@@ -1,6 +1,7 @@
-// calibrate_kernels.cuh -- register-only FP32 FMA loops that measure the denominator of the "alu" roofline
-// (DESIGN.md 6.1): MEASURED_PEAKS.json carries HBM and bf16 figures but no FP32 one, so the library can
-// time the plain-ALU peak itself on the device it runs on.  PACKED = 0: scalar FFMA; 1: FFMA2 (f32x2).
+// probe_kernels.cuh -- kernels of libcolatus_probe (include/colatus_probe.h), NOT of the product library.
+// Register-only FP32 FMA loops that measure the denominator of the "alu" roofline:
+// MEASURED_PEAKS.json carries HBM and bf16 figures but no FP32 one, so the plain-ALU peak is timed on the
+// device itself.  PACKED = 0: scalar FFMA; 1: FFMA2 (f32x2).
 // Each thread runs CHAINS independent dependent chains x = x * a + b, so the pipe is limited by issue,
 // not latency; 2 flop per lane-FMA.  The result is stored only if it is NaN-like, which never happens
 // for the chosen constants, but keeps the loop alive.
@@ -61,9 +62,13 @@ __global__ void __launch_bounds__(CAL_THREADS) calibrate_fma_kernel(float a, flo
 // Register-only loops whose body is one "group" of 12 packed FP32 ops (the FP work of one packed
 // pair-interaction) plus, per MODE, the extra instructions whose cost next to a saturated FMA pipe is in
 // question.  The caller converts the launch time into SMSP cycles per group.
-//   0: 12 FFMA2 (two shared operands)            3: 12 FFMA2 with three distinct 64-bit register operands
-//   1: 12 FFMA2 + 2 MUFU.RSQ                      4: 12 FFMA2 + 1 LDS.128 (broadcast address)
-//   2: 12 FFMA2 + 2 IADD                          5: 24 scalar FFMA + 2 MUFU.RSQ
+//   0: 12 FFMA2 x = x*A + B (two loop-constant operands)
+//   1: 0 + 2 MUFU.RSQ                              2: 0 + 2 IADD
+//   3: 12 accumulates a[t][c] = w[t]*d[t][c] + a[t][c], t-major: triples that share w (three distinct 64-bit
+//      register operands each; the operand-reuse cache can hold w for the 2nd and 3rd of a triple)
+//   4: 0 + 1 LDS.128 (broadcast address)           5: 24 scalar FFMA + 2 MUFU.RSQ
+//   6: the accumulates of 3, c-major: w changes every instruction, no operand reuse possible
+//   7: 0 + 6 DFMA (does the FP64 pipe run next to a saturated FP32 pipe?)
 constexpr int PROBE_GROUPS = 2048;   // groups per warp
 
 template <int MODE>
@@ -71,17 +76,27 @@ __global__ void __launch_bounds__(CAL_THREADS) pipe_probe_kernel(float a, float 
     __shared__ float4 tile[64];
     if (threadIdx.x < 64) tile[threadIdx.x] = make_float4(a, b, a, b);
     __syncthreads();
-    u64 x[CAL_CHAINS], y[CAL_CHAINS], z[CAL_CHAINS];
+    u64 w[4], d[4][3], acc[4][3];
     float xs[2 * CAL_CHAINS];
+    double y[6];
     const u64 A = pack2(a, a), Bv = pack2(b, b);
+    const double da = a, db = b;
 #pragma unroll
     for (int c = 0; c < CAL_CHAINS; ++c) {
-        x[c] = pack2((float)threadIdx.x + c, (float)blockIdx.x - c);
-        y[c] = pack2(b * (c + 1), b * (c + 2));
-        z[c] = pack2(a - 1e-3f * c, a - 2e-3f * c);
         xs[2 * c] = (float)threadIdx.x + c;
         xs[2 * c + 1] = (float)blockIdx.x - c;
     }
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+        w[t] = pack2(a * (t + 1) * 1e-3f, b * (t + 2) * 1e-3f);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            d[t][c] = pack2(a + 0.01f * (t * 3 + c) + threadIdx.x * 1e-6f, b - 0.02f * (t * 3 + c));
+            acc[t][c] = pack2((float)threadIdx.x, (float)blockIdx.x + c + t);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) y[c] = (double)threadIdx.x + c;
     float r0 = 1.5f + threadIdx.x, r1 = 2.5f + threadIdx.x;
     int k0 = threadIdx.x, k1 = blockIdx.x | 1;
     const uint32_t tile_addr = smem_u32(tile);
@@ -92,11 +107,21 @@ __global__ void __launch_bounds__(CAL_THREADS) pipe_probe_kernel(float a, float 
             if (MODE == 5) {
 #pragma unroll
                 for (int c = 0; c < 24; ++c) xs[c % (2 * CAL_CHAINS)] = fmaf(xs[c % (2 * CAL_CHAINS)], a, b);
+            } else if (MODE == 3) {
+#pragma unroll
+                for (int t = 0; t < 4; ++t)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) acc[t][c] = fma2(w[t], d[t][c], acc[t][c]);
+            } else if (MODE == 6) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) acc[t][c] = fma2(w[t], d[t][c], acc[t][c]);
             } else {
 #pragma unroll
-                for (int c = 0; c < 12; ++c) {
-                    const int q = c % CAL_CHAINS;
-                    x[q] = MODE == 3 ? fma2(x[q], z[q], y[q]) : fma2(x[q], A, Bv);
+                for (int c = 0; c < 12; ++c) {                 // 12 independent chains
+                    acc[c / 3][c % 3] = fma2(acc[c / 3][c % 3], A, Bv);
+                    if (MODE == 7 && c < 6) y[c] = fma(y[c], da, db);
                 }
             }
             if (MODE == 1 || MODE == 5) {
@@ -109,7 +134,7 @@ __global__ void __launch_bounds__(CAL_THREADS) pipe_probe_kernel(float a, float 
             }
             if (MODE == 4) {
                 float v0, v1, v2, v3;
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
                              : "=f"(v0), "=f"(v1), "=f"(v2), "=f"(v3)
                              : "r"(tile_addr + ((it & 31) << 4)));
             }
@@ -117,11 +142,17 @@ __global__ void __launch_bounds__(CAL_THREADS) pipe_probe_kernel(float a, float 
     }
     float s = r0 + r1 + (float)(k0 ^ k1);
 #pragma unroll
-    for (int c = 0; c < CAL_CHAINS; ++c) {
-        float lo, hi;
-        unpack2(x[c], lo, hi);
-        s += lo + hi + xs[2 * c] + xs[2 * c + 1];
-    }
+    for (int c = 0; c < 2 * CAL_CHAINS; ++c) s += xs[c];
+#pragma unroll
+    for (int t = 0; t < 4; ++t)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            float lo, hi;
+            unpack2(acc[t][c], lo, hi);
+            s += lo + hi;
+        }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) s += (float)y[c];
     if (s == 123456.789f) sink[0] = s;
 }
 

@@ -2,16 +2,24 @@
 
 Eq. (1) shards by TARGETS: every rank holds all n sources, owns a contiguous slice of the
 particles, evaluates forces / drifts / kicks for its slice only (libcolatus target range) and the
-ranks exchange updated positions with one all-gather after each drift -- the path's only real
-exchange step.  One process per GPU; `torch.distributed` (NCCL over NVLink on GPUs, gloo in the
-CPU tests) is the plumbing.
+ranks exchange updated positions with ONE all-gather per step, after the first half drift -- the
+path's only real exchange step (it replaces the paper's per-step device-to-host copy of everything,
+PAPER.md:116).  After the kick-drift a rank's copy of the OTHER slices is stale; nothing needs them
+until the next step's all-gather, so the stepper only marks the positions dirty and gathers lazily
+before a read of full positions (`sync_positions`: download, potential energy).  Diagnostics are one
+all-reduce of 16 doubles; a tracer's velocity row is recorded by the rank that owns the particle and
+the rows are assembled on read.  One process per GPU; `torch.distributed` (NCCL over NVLink on GPUs,
+gloo in the CPU tests) is the plumbing.
 
 `ShardedStepper` holds only the host-side sequencing.  The per-slice work is done by an `ops`
 object: `LibcolatusOps` (the product: calls the C ABI) or, in tests/, a stand-in that lets the
-sequencing be checked on CPU without a GPU.
+sequencing be checked on CPU without a GPU.  An `ops` object provides
+    drift(d); force_kick_drift(cv, ck, d2); diagnostics(a, with_potential) -> 16 doubles over the slice;
+    trace_rows(first_step, n_steps) -> float32 [n_steps, k, 4] of this rank's ring (optional).
 """
 from __future__ import annotations
 
+import numpy as np
 import torch
 import torch.distributed as dist
 
@@ -30,6 +38,7 @@ class LibcolatusOps:
     def __init__(self, pos, vel, acc_slice, n, eps2, begin, count):
         from . import binding as B
         self.B = B
+        self.trace_k = 0
         B.colatus_upload(pos, vel, acc_slice, n, eps2)
         B.colatus_set_target_range(begin, count)
 
@@ -39,20 +48,38 @@ class LibcolatusOps:
     def force_kick_drift(self, cv, ck, d2):
         self.B.colatus_force_kick_drift(cv, ck, d2)
 
+    def diagnostics(self, a, with_potential=False):
+        return self.B.colatus_diagnostics(a, with_potential)
+
+    def trace(self, idx_dev, ring_dev, capacity_steps):
+        """idx_dev: int32 device tensor [k] (global particle indices); ring_dev: float32 device tensor
+        [capacity_steps, k, 4].  Only the tracers inside this rank's slice are ever written."""
+        self.trace_k = int(idx_dev.numel())
+        self.B.colatus_trace(idx_dev, self.trace_k, ring_dev, capacity_steps)
+
+    def trace_rows(self, first_step, n_steps):
+        out = np.empty((n_steps, self.trace_k, 4), dtype=np.float32)
+        self.B.colatus_trace_read(out, first_step, n_steps)
+        return out
+
 
 class ShardedStepper:
     def __init__(self, pos: torch.Tensor, n: int, ops, group=None):
         self.world = dist.get_world_size(group) if dist.is_initialized() else 1
         self.rank = dist.get_rank(group) if dist.is_initialized() else 0
         self.group = group
-        self.pos = pos                       # [n,4] full body array, identical on all ranks at step ends
+        self.pos = pos                       # [n,4] full body array; other ranks' slices may be stale (dirty)
         self.n = n
         self.begin, self.count = partition(n, self.world, self.rank)
         self.ops = ops
+        self.dirty = False                   # True: the slices owned by other ranks are not current here
+        self.gathers = 0                     # all-gathers issued (one per step + lazy syncs)
 
     def _allgather_positions(self):
+        self.dirty = False
         if self.world == 1:
             return
+        self.gathers += 1
         mine = self.pos[self.begin:self.begin + self.count]
         if self.pos.is_cuda:
             dist.all_gather_into_tensor(self.pos, mine, group=self.group)      # in place (NCCL)
@@ -62,14 +89,52 @@ class ShardedStepper:
             for r, p in enumerate(parts):
                 self.pos[r * self.count:(r + 1) * self.count].copy_(p)
 
+    def sync_positions(self):
+        """Make every rank's full position array current (no-op unless a step has run since the last gather)."""
+        if self.dirty:
+            self._allgather_positions()
+
     def step_coeffs(self, d1, cv, ck, d2):
-        """x += d1 v | all-gather x | F, v = cv v + ck F, x += d2 v | all-gather x."""
+        """x += d1 v (own slice) | all-gather x | F, v = cv v + ck F, x += d2 v (own slice)."""
         self.ops.drift(d1)
         self._allgather_positions()
         self.ops.force_kick_drift(cv, ck, d2)
-        self._allgather_positions()
+        self.dirty = self.world > 1
 
     def step(self, tau, a, H):
         """Eqs. (3)-(5), with the coefficients libcolatus forms."""
         from . import binding as B
         self.step_coeffs(*B.colatus_step_coefficients(tau, a, H))
+
+    def diagnostics(self, a, with_potential=False):
+        """colatus_diagnostics over all n bodies: every rank reduces its own slice (out[0..8], out[13..15] are
+        additive over slices), then ONE all-reduce of the 16 doubles; centre of mass = sum m x / M afterwards.
+        W needs every rank's sources to be current, so the positions are synchronised first."""
+        if with_potential:
+            self.sync_positions()
+        d = np.array(self.ops.diagnostics(a, with_potential), dtype=np.float64)
+        step = d[12]
+        if self.world > 1:
+            t = torch.from_numpy(d.copy())
+            if self.pos.is_cuda:
+                t = t.to(self.pos.device)
+            dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+            d = t.cpu().numpy()
+        d[9:12] = d[13:16] / d[0]
+        d[12] = step
+        return d
+
+    def trace_read(self, idx, first_step, n_steps):
+        """Rows [first_step, +n_steps) of the tracer record, float32 [n_steps, k, 4], assembled from the ranks
+        that own each tracer (idx: the global particle indices given to `ops.trace`)."""
+        rows = self.ops.trace_rows(first_step, n_steps)
+        if self.world == 1:
+            return rows
+        idx = np.asarray(idx, dtype=np.int64)
+        mine = (idx >= self.begin) & (idx < self.begin + self.count)
+        rows = np.where(mine[None, :, None], rows, np.float32(0.0))            # exact: owners' values + zeros
+        t = torch.from_numpy(np.ascontiguousarray(rows))
+        if self.pos.is_cuda:
+            t = t.to(self.pos.device)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+        return t.cpu().numpy()

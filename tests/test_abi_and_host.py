@@ -30,6 +30,22 @@ def test_every_declared_symbol_is_exported_and_bound():
     assert declared == set(B.SIGNATURES), declared ^ set(B.SIGNATURES)
 
 
+def test_probe_library_is_separate_and_exports_its_header():
+    """Microbenchmarks live in libcolatus_probe.so (include/colatus_probe.h), not in the product ABI."""
+    from paper_1208_3444_b200 import probe as P
+    header = open(os.path.join(ROOT, "include", "colatus_probe.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(colatus_probe_[a-z_0-9]+)\s*\(", header))
+    assert declared == set(P.SIGNATURES) and len(declared) == 2
+    handle = P.lib()
+    for name in declared:
+        assert hasattr(handle, name)
+    import subprocess
+    product = subprocess.check_output(["nm", "-D", "--defined-only", B.LIB_PATH], text=True)
+    assert "probe" not in product and "calibrate" not in product
+    assert P.lib().colatus_probe_pipe(0, 99, None) == -1           # argument check needs no device
+
+
 def test_library_does_not_link_torch_or_oracle():
     import subprocess
     out = subprocess.check_output(["ldd", B.LIB_PATH], text=True)

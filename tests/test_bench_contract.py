@@ -42,3 +42,20 @@ def test_reference_arm_under_torchrun_env_only_rank0_prints():
                         "--steps", "1", "--warmup", "0", "--n", "4096"], capture_output=True, text=True, cwd=ROOT,
                        env=env, timeout=600)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_native_arm_with_more_gpus_than_the_box_has_fails_loudly():
+    """`python bench.py --gpus N` (no torchrun) starts N ranks itself; with fewer than N devices it must refuse
+    instead of timing one GPU and printing n_gpus: 1 (round-1 finding)."""
+    import torch
+    need = torch.cuda.device_count() + 2
+    r = _run("--gpus", str(need), "--steps", "1", "--warmup", "0")
+    assert r.returncode != 0
+    assert "refusing to run fewer ranks" in (r.stderr + r.stdout)
+
+
+def test_native_arm_rejects_a_world_size_that_contradicts_gpus():
+    env = dict(os.environ, RANK="0", WORLD_SIZE="2", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, cwd=ROOT, env=env, timeout=600)
+    assert r.returncode != 0 and "WORLD_SIZE=2" in (r.stderr + r.stdout)

@@ -1,0 +1,99 @@
+"""The target-sharded driver (paper_1208_3444_b200/sharded.py) on the GPU through the C ABI:
+ShardedStepper + LibcolatusOps at world size 1 (no process group -- one GPU is all this box has) must reproduce
+the oracle's trajectory, diagnostics and tracer record like the single-GPU path does.  The exchange step itself
+(all-gather / all-reduce sequencing at world size 2) is covered on CPU by tests/test_sharded_gloo.py."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+from paper_1208_3444_b200 import binding as B  # noqa: E402
+from paper_1208_3444_b200 import inputs  # noqa: E402
+
+
+def test_sharded_stepper_world1_matches_oracle():
+    import torch
+    from paper_1208_3444_b200.harness import Session
+    from paper_1208_3444_b200.sharded import LibcolatusOps, ShardedStepper
+    cfg, pm, vel = inputs.make_config(1)
+    steps = 10
+    tr = np.arange(0, cfg.n, cfg.n // 16, dtype=np.int32)
+    with Session(cfg.G, cfg.n) as s:
+        pos, v = s.to_device(pm), s.to_device(vel)
+        acc = torch.zeros_like(pos)
+        ops = LibcolatusOps(pos, v, acc, cfg.n, cfg.eps2, 0, cfg.n)
+        stepper = ShardedStepper(pos, cfg.n, ops)
+        assert (stepper.world, stepper.begin, stepper.count) == (1, 0, cfg.n)
+        idx = torch.from_numpy(tr).to(pos.device)
+        ring = torch.zeros((steps, tr.size, 4), dtype=torch.float32, device=pos.device)
+        ops.trace(idx, ring, steps)
+        mids, ends = oracle.midstep_schedule(cfg.cosmo, cfg.a_start, cfg.tau, steps)
+        for a, H in mids:
+            stepper.step(cfg.tau, a, H)
+        assert stepper.gathers == 0 and not stepper.dirty
+        d = stepper.diagnostics(ends[-1], with_potential=True)
+        rows = stepper.trace_read(tr, 0, steps)
+        torch.cuda.synchronize()
+        x_gpu, v_gpu = pos.cpu().numpy(), v.cpu().numpy()
+    st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+    rows_ref = np.zeros((steps, tr.size, 3))
+    for n, (a, H) in enumerate(mids):
+        st.step(cfg.tau, a, H)
+        rows_ref[n] = st.v[tr]
+    assert np.linalg.norm(x_gpu[:, :3].astype(np.float64) - st.x, axis=1).max() <= 1e-5          # G16
+    dref = st.diagnostics(ends[-1], with_potential=True)
+    assert d[0] == pytest.approx(dref[0], rel=1e-6) and d[7] == pytest.approx(dref[7], rel=1e-4)
+    assert d[8] == pytest.approx(dref[8], rel=1e-5) and d[12] == steps
+    assert np.allclose(d[9:12], dref[9:12], atol=2e-6) and np.allclose(d[13:16], d[9:12] * d[0], rtol=1e-12)
+    assert np.array_equal(rows[-1, :, :3], v_gpu[tr, :3])                                        # bit-exact record
+    vr = np.sqrt((rows_ref ** 2).sum(2).mean())
+    assert np.abs(rows[:, :, :3] - rows_ref).max() <= 2e-4 * vr
+
+
+def test_sharded_two_slices_evaluated_one_after_the_other_equal_the_full_step():
+    """What rank 0 and rank 1 of a 2-GPU run would each compute, done one after the other on this GPU (no
+    kernel waits on another): drift / force-kick-drift restricted to a slice touch that slice only, and the two
+    slices together equal the unsharded step up to the summation order (the source split is chosen per target
+    count, reading G14)."""
+    import torch
+    from paper_1208_3444_b200.harness import Session
+    cfg, pm, vel = inputs.make_config(1)
+    rng = np.random.Generator(np.random.PCG64(5))
+    vel = vel.copy()
+    vel[:, :3] = 0.05 * rng.standard_normal((cfg.n, 3)).astype(np.float32)
+    c = B.colatus_step_coefficients(cfg.tau, 0.05, 3.0)
+    half = cfg.n // 2
+    with Session(cfg.G, cfg.n) as s:
+        # reference: whole range through the same separate kernels (drift, force, kick-drift)
+        s.upload(pm, vel, cfg.eps2)
+        B.colatus_set_target_range(0, cfg.n)
+        B.colatus_drift(c[0])
+        B.colatus_force_kick_drift(c[1], c[2], c[3])
+        x_ref, v_ref = s.download()
+        # "two ranks": both drift their slice of the same start state, the drifted slices are exchanged
+        # (here: they already sit in the one array), then each force-kick-drifts its slice from a copy of the
+        # gathered positions
+        s.upload(pm, vel, cfg.eps2)
+        for b in (0, half):
+            B.colatus_set_target_range(b, half)
+            B.colatus_drift(c[0])
+        torch.cuda.synchronize()
+        gathered = s.pos.clone()
+        out_x, out_v = np.empty_like(pm), np.empty_like(vel)
+        for b in (0, half):
+            s.pos.copy_(gathered)
+            acc = torch.zeros((half, 4), dtype=torch.float32, device=s.pos.device)
+            B.colatus_upload(s.pos, s.vel, acc, cfg.n, cfg.eps2)
+            B.colatus_set_target_range(b, half)
+            B.colatus_force_kick_drift(c[1], c[2], c[3])
+            x, v = s.download()
+            other = slice(half, cfg.n) if b == 0 else slice(0, half)
+            assert np.array_equal(x[other], gathered.cpu().numpy()[other])          # other slice untouched
+            out_x[b:b + half], out_v[b:b + half] = x[b:b + half], v[b:b + half]
+            s.vel.copy_(s.to_device(vel))                                            # rank-local velocities
+    assert np.array_equal(out_x[:, 3], x_ref[:, 3])
+    vr = float(np.sqrt((v_ref[:, :3].astype(np.float64) ** 2).sum(1).mean()))
+    assert np.abs(out_v[:, :3] - v_ref[:, :3]).max() <= 2e-5 * vr
+    assert np.abs(out_x[:, :3] - x_ref[:, :3]).max() <= 1e-6
+    assert not np.array_equal(out_x[:, :3], pm[:, :3])

@@ -107,6 +107,46 @@ def test_static_energy_conservation_and_potential():
     assert d1[7] > 1e-4 * abs(E0)                                      # something happened
 
 
+def test_layzer_irvine_on_the_gpu():
+    """P11 on the GPU (tier T3): with T = 1/2 sum m a^2 v^2 and W from the potential-fused force pass,
+    eqs. (1), (3)-(5) and (7) imply d(T+W)/dt = -H (2T + W).  Config 1 (EdS), a fixed time span covered in 40 and
+    in 80 steps, colatus_diagnostics(with_potential) at every step end: the trapezoid-integrated residual is far
+    below |Delta E| and shrinks ~4x when tau halves (the scheme is second order), and T, W follow the oracle's."""
+    cfg, pm, vel = inputs.make_config(1)
+    span = 0.004
+    res, dE = [], []
+    for steps in (40, 80):
+        tau = span / steps
+        mids, ends = oracle.midstep_schedule(cfg.cosmo, cfg.a_start, tau, steps)
+        st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+        with _session(cfg.G, cfg.n) as s:
+            s.upload(pm, vel, cfg.eps2)
+            d = s.diagnostics(ends[0], True)
+            E = [d[7] + d[8]]
+            rhs = [B.colatus_hubble(cfg.cosmo, ends[0]) * (2 * d[7] + d[8])]
+            a = cfg.a_start
+            for i in range(steps):
+                a_mid = B.colatus_a_advance(cfg.cosmo, a, 0.5 * tau)
+                B.colatus_step(tau, a_mid, B.colatus_hubble(cfg.cosmo, a_mid))
+                a = B.colatus_a_advance(cfg.cosmo, a_mid, 0.5 * tau)
+                assert a == pytest.approx(ends[i + 1], rel=1e-9)
+                d = s.diagnostics(a, True)
+                E.append(d[7] + d[8])
+                rhs.append(B.colatus_hubble(cfg.cosmo, a) * (2 * d[7] + d[8]))
+                st.step(tau, *mids[i])
+                r = st.diagnostics(ends[i + 1], True)
+                assert d[8] == pytest.approx(r[8], rel=1e-4), (steps, i)
+                assert abs(d[7] - r[7]) <= 1e-4 * abs(r[8]), (steps, i)        # T starts at 0: scale by |W|
+        rhs = np.array(rhs)
+        integral = tau * (rhs.sum() - 0.5 * (rhs[0] + rhs[-1]))                # trapezoid
+        res.append(abs(E[-1] - E[0] + integral))
+        dE.append(abs(E[-1] - E[0]))
+        assert res[-1] <= 1e-2 * dE[-1], (steps, res, dE)
+    record_parity("Layzer-Irvine on the GPU (config 1, 40 / 80 steps)", residual_40=res[0], residual_80=res[1],
+                  delta_E=dE[1])
+    assert res[0] / res[1] == pytest.approx(4.0, rel=0.35), res
+
+
 def test_step_coeffs_equals_step_and_is_reproducible():
     cfg, pm, vel = inputs.make_config(1)
     out = []

@@ -1,6 +1,8 @@
 """World-size-2 CPU test (gloo) of the target-sharded multi-GPU sequencing (DESIGN.md "Multi-GPU",
 SURVEY 8e): ShardedStepper must drift / force-kick-drift only its own slice, all-gather positions
-after every drift, and reproduce the single-process trajectory exactly.
+ONCE per step (after the first drift; lazily before a read of full positions), reduce the diagnostics
+with one all-reduce, assemble the tracer rows from the owning ranks, and reproduce the single-process
+trajectory exactly.
 
 No GPU here, so the per-slice work is done by a stand-in `ops` built on the FP64 oracle (tests may
 use the oracle); what is under test is the host-side sequencing and the exchange step in
@@ -24,14 +26,21 @@ from paper_1208_3444_b200.sharded import ShardedStepper, partition
 N, STEPS, WORLD = 512, 4, 2
 
 
+TRACERS = np.array([3, 100, 255, 256, 400, 511], dtype=np.int64)     # both slices, including their edges
+
+
 class OracleSliceOps:
-    """Drift / force+kick+drift of eqs. (3)-(5) on the slice [begin, begin+count) of float64 state.
+    """Drift / force+kick+drift of eqs. (3)-(5) on the slice [begin, begin+count) of float64 state, the
+    slice diagnostics in colatus_diagnostics' layout, and a tracer ring that (like libcolatus with a target
+    range) records only the tracers this rank owns.
 
     `pos` is the [n,4] float64 tensor ShardedStepper all-gathers; velocities exist for the slice only."""
 
-    def __init__(self, pos, vel_slice, eps2, G, begin, count):
+    def __init__(self, pos, vel_slice, eps2, G, begin, count, steps):
         self.pos, self.vel, self.eps2, self.G = pos, vel_slice, eps2, G
         self.begin, self.count = begin, count
+        self.step = 0
+        self.ring = np.zeros((steps, TRACERS.size, 4), dtype=np.float32)
 
     def drift(self, d):
         s = slice(self.begin, self.begin + self.count)
@@ -45,6 +54,32 @@ class OracleSliceOps:
         self.vel.mul_(cv).add_(ck * F)
         s = slice(self.begin, self.begin + self.count)
         self.pos[s, :3] += d2 * self.vel
+        for t, k in enumerate(TRACERS):
+            if self.begin <= k < self.begin + self.count:
+                self.ring[self.step, t, :3] = self.vel[k - self.begin].numpy()
+                self.ring[self.step, t, 3] = 1.0
+        self.step += 1
+
+    def diagnostics(self, a, with_potential=False):
+        s = slice(self.begin, self.begin + self.count)
+        x, m, v = self.pos[s, :3].numpy(), self.pos[s, 3].numpy(), self.vel.numpy()
+        out = np.zeros(16)
+        out[0] = m.sum()
+        out[1:4] = (m[:, None] * v).sum(0)
+        out[4:7] = a * a * out[1:4]
+        out[7] = 0.5 * a * a * (m * (v * v).sum(1)).sum()
+        out[8] = np.nan
+        if with_potential:
+            targets = np.arange(self.begin, self.begin + self.count, dtype=np.int64)
+            _, phi = oracle.forces_xm(self.pos[:, :3].numpy(), self.pos[:, 3].numpy(), self.eps2, self.G, targets, True)
+            out[8] = 0.5 * (m * phi).sum() / a
+        out[13:16] = (m[:, None] * x).sum(0)
+        out[9:12] = out[13:16] / out[0]
+        out[12] = self.step
+        return out
+
+    def trace_rows(self, first_step, n_steps):
+        return self.ring[first_step:first_step + n_steps].copy()
 
 
 def _free_port():
@@ -61,12 +96,24 @@ def _worker(rank, world, port, pm, vel, eps2, G, coeffs, out_dir):
         pos = torch.from_numpy(pm.astype(np.float64))
         begin, count = partition(pm.shape[0], world, rank)
         v = torch.from_numpy(vel[begin:begin + count, :3].astype(np.float64))
-        stepper = ShardedStepper(pos, pm.shape[0], OracleSliceOps(pos, v, eps2, G, begin, count))
+        stepper = ShardedStepper(pos, pm.shape[0], OracleSliceOps(pos, v, eps2, G, begin, count, len(coeffs)))
         assert (stepper.begin, stepper.count) == (begin, count)
         for c in coeffs:
             stepper.step_coeffs(*c)
+        assert stepper.gathers == len(coeffs) and stepper.dirty          # ONE all-gather per step
+        other = slice(0, count) if rank == 1 else slice(count, 2 * count)
+        stale = pos[other].clone()
+        d_kin = stepper.diagnostics(0.5)                                  # no potential: no gather needed
+        assert stepper.gathers == len(coeffs) and torch.equal(pos[other], stale)
+        d_pot = stepper.diagnostics(0.5, with_potential=True)             # W reads all sources: lazy gather
+        assert stepper.gathers == len(coeffs) + 1 and not stepper.dirty and not torch.equal(pos[other], stale)
+        stepper.sync_positions()
+        assert stepper.gathers == len(coeffs) + 1                         # already current
+        rows = stepper.trace_read(TRACERS, 0, len(coeffs))
         np.save(os.path.join(out_dir, f"pos{rank}.npy"), pos.numpy())
         np.save(os.path.join(out_dir, f"vel{rank}.npy"), v.numpy())
+        np.save(os.path.join(out_dir, f"diag{rank}.npy"), np.stack([d_kin, d_pot]))
+        np.save(os.path.join(out_dir, f"rows{rank}.npy"), rows)
     finally:
         dist.destroy_process_group()
 
@@ -92,8 +139,11 @@ def test_two_rank_sharded_stepping_matches_single_process(tmp_path):
              nprocs=WORLD, join=True)
 
     ref = oracle.State(pm, vel, cfg.eps2, cfg.G)
-    for c in coeffs:
+    rows_ref = np.zeros((STEPS, TRACERS.size, 4), dtype=np.float32)
+    for n, c in enumerate(coeffs):
         ref.step_coeffs(*c)
+        rows_ref[n, :, :3] = ref.v[TRACERS]
+        rows_ref[n, :, 3] = 1.0
     pos0 = np.load(tmp_path / "pos0.npy")
     pos1 = np.load(tmp_path / "pos1.npy")
     assert np.array_equal(pos0, pos1)                      # every rank ends with the same full position array
@@ -101,3 +151,17 @@ def test_two_rank_sharded_stepping_matches_single_process(tmp_path):
     v = np.concatenate([np.load(tmp_path / "vel0.npy"), np.load(tmp_path / "vel1.npy")])
     assert np.abs(v - ref.v).max() <= 1e-13
     assert np.array_equal(pos0[:, 3], pm[:, 3].astype(np.float64))   # masses untouched by the exchange
+
+    # diagnostics: one all-reduce of the 16 doubles gives the whole-system sums on every rank
+    d0, d1 = np.load(tmp_path / "diag0.npy"), np.load(tmp_path / "diag1.npy")
+    assert np.array_equal(d0[1], d1[1]) and np.array_equal(d0[0, :8], d1[0, :8])
+    dref = ref.diagnostics(0.5, with_potential=True)
+    for i in range(0, 12):
+        assert d0[1][i] == pytest.approx(dref[i], rel=1e-12, abs=1e-15), i
+    assert d0[1][13:16] == pytest.approx(dref[9:12] * dref[0], rel=1e-12)       # sum m x (additive over shards)
+    assert np.isnan(d0[0][8]) and d0[0][7] == pytest.approx(dref[7], rel=1e-12)
+    assert d0[1][12] == STEPS
+    # tracers: each row comes from the rank that owns the particle; both ranks assemble the same full record
+    r0, r1 = np.load(tmp_path / "rows0.npy"), np.load(tmp_path / "rows1.npy")
+    assert np.array_equal(r0, r1)
+    assert np.array_equal(r0[:, :, 3], rows_ref[:, :, 3]) and np.abs(r0[:, :, :3] - rows_ref[:, :, :3]).max() <= 1e-7 * np.abs(rows_ref).max()
