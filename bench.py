@@ -312,7 +312,7 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
                 "traffic_from": cap["profile"] if traffic else None,
                 "algorithmic_bytes": 16 * n * (2 + (geo["source_splits"] if geo["source_splits"] > 1 else 0)),
                 "kernel": "force_kernel<%d,%d,4,false,2>%s" % (geo["targets_per_thread"] // 2,
-                                                                 {6: 512, 4: 512, 2: 256}[geo["targets_per_thread"]],
+                                                                 {6: 512, 4: 512, 2: 128}[geo["targets_per_thread"]],
                                                                  " equal-mass loop" if equal_mass else ""),
                 "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / ms_step,

@@ -276,7 +276,7 @@ int64_t  colatus_launch_count(void);
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 
 /* Tuning overrides for measurements (0 restores the automatic choice):
- *   "targets_per_thread" in {0,2,4,6};  "source_splits" in [0,16]. */
+ *   "targets_per_thread" in {0,2,4,6};  "source_splits" in [0,64] (capped at 16 above 65536 bodies). */
 int colatus_set_option(const char *name, int64_t value);
 
 const char *colatus_last_error(void);

@@ -20,11 +20,14 @@ namespace {
 
 using namespace colatus;
 
-constexpr int MAX_SPLITS = REDUCE_MAX_SPLITS;   // source splits (partials kept in the workspace)
+constexpr int MAX_SPLITS = REDUCE_MAX_SPLITS;   // source splits (partials kept in the workspace): small problems
+constexpr int MAX_SPLITS_LARGE = 16;            // ... and problems above SMALL_N bodies (bounds the partials' memory)
+constexpr int64_t SMALL_N = 65536;
 constexpr int NSTAGES = 4;            // shared-memory ring depth
 constexpr int DIAG_BLOCKS_MAX = 1024;
 constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
 constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in colatus_run
+constexpr int GRAPH_STEPS = 8;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
 
 struct Geometry {
     int IP = 0, TJ = 0;   // target pairs per thread, sources per tile
@@ -70,10 +73,11 @@ struct Context {
     // colatus_run: private capture stream, ordering events, cached one-step graph
     cudaStream_t run_stream = nullptr;
     cudaEvent_t run_ev_in = nullptr, run_ev_out = nullptr;
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t graph_exec = nullptr;
+    cudaGraph_t graph = nullptr, graph_k = nullptr;           // one step / GRAPH_STEPS steps
+    cudaGraphExec_t graph_exec = nullptr, graph_exec_k = nullptr;
     bool graph_valid = false;
     int64_t graph_launches = 0;
+    int graph_generation = 0;   // equal-mass stamp baked into the captured kernels
     char err[512] = "";
 };
 
@@ -95,8 +99,27 @@ int fail(int code, const char *fmt, ...) {
                         __FILE__, __LINE__);                                                        \
     } while (0)
 
+// Kernel launch with the programmatic-stream-serialization attribute (pdl): the kernel may be scheduled before its
+// predecessor in the stream has drained and synchronises with griddepcontrol.wait (force_kernels.cuh).
+template <typename... KArgs, typename... Args>
+cudaError_t launch_ex(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                      Args &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline int max_splits(int64_t n) { return n <= SMALL_N ? MAX_SPLITS : MAX_SPLITS_LARGE; }
 
 Workspace workspace_layout(int64_t n_max) {
     Workspace w;
@@ -104,7 +127,7 @@ Workspace workspace_layout(int64_t n_max) {
     const size_t n_pad = round_up(n, (size_t)PAD_SOURCES) + (size_t)MAX_SPLITS * PAD_SOURCES;
     size_t off = 256;                        // [0, 256): mass_flag (zeroed by colatus_init)
     w.packed = off;      off += round_up(n_pad * 16, 256);
-    w.partials = off;    off += round_up((size_t)MAX_SPLITS * n * 16, 256);
+    w.partials = off;    off += round_up((size_t)max_splits(n_max) * n * 16, 256);
     w.scratch_acc = off; off += round_up(n * 16, 256);
     w.trace_slot = off;  off += round_up(n * 4, 256);
     w.diag = off;        off += round_up((size_t)(DIAG_BLOCKS_MAX + 2) * DIAG_Q * 8, 256);
@@ -125,7 +148,7 @@ Workspace workspace_layout(int64_t n_max) {
 // target pair of a CTA with the SM to itself, c0 = per-CTA prologue/epilogue.  Pure function of
 // (n, t_count, SM count): the geometry, and with it the summation order, is reproducible.
 Geometry choose_geometry(int64_t n, int64_t t_count) {
-    static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 256}};   // (target pairs per thread, tile)
+    static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 128}};   // (target pairs per thread, tile)
     static const double a_us[4] = {0.0, 0.0295, 0.0287, 0.0274};        // per source, per target pair
     const double c0_us = 0.77, ramp = 0.096;
     Geometry best;
@@ -136,7 +159,11 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
         const int64_t per_cta = (int64_t)FORCE_THREADS * 2 * IP;
         const int64_t tiles_t = (t_count + per_cta - 1) / per_cta;
         const int64_t src_tiles = (n + TJ - 1) / TJ;
-        const int64_t smax = src_tiles < MAX_SPLITS ? src_tiles : MAX_SPLITS;
+        // automatic choice: at most 16 splits -- the sweep (profiles/r02_geometry_sweep.md) shows that beyond 16 the
+        // growing partial-sum reduction eats what the force kernel gains (<= 1.8 % at best, -35 % at worst);
+        // a forced split count (colatus_set_option) may go up to max_splits(n)
+        const int64_t cap = g.force_splits ? max_splits(n) : MAX_SPLITS_LARGE;
+        const int64_t smax = src_tiles < cap ? src_tiles : cap;
         for (int64_t s = 1; s <= smax; ++s) {
             if (g.force_splits && s != g.force_splits && g.force_splits <= smax) continue;
             const int64_t tps = (src_tiles + s - 1) / s;
@@ -160,7 +187,8 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
 template <int IP, int TJ, bool POT>
 cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
                                  int64_t t_count, float eps2, float scale, int final_out, float4 *out,
-                                 int64_t out_stride, const int *mass_flag, int generation, cudaStream_t st) {
+                                 int64_t out_stride, const int *mass_flag, int generation, int *step_ctr,
+                                 cudaStream_t st, bool pdl) {
     auto kern = force_kernel<IP, TJ, NSTAGES, POT, 2>;
     const size_t smem = force_smem_bytes<IP, TJ, NSTAGES, POT>();
     static int attr_epoch = 0;            // function attributes are per device: set again after every colatus_init
@@ -170,25 +198,24 @@ cudaError_t launch_force_variant(const Geometry &geo, const float4 *pos_mass, co
         attr_epoch = g.init_epoch;
     }
     dim3 grid((unsigned)geo.tiles_t, (unsigned)geo.splits);
-    kern<<<grid, FORCE_THREADS, smem, st>>>(pos_mass, packed, t_begin, t_count, geo.tiles_per_split, eps2, scale,
-                                            final_out, out, out_stride, mass_flag, generation);
-    return cudaGetLastError();
+    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, pos_mass, packed, t_begin, t_count,
+                     geo.tiles_per_split, eps2, scale, final_out, out, out_stride, mass_flag, generation, step_ctr);
 }
 
 template <bool POT>
 cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const float4 *packed, int64_t t_begin,
                          int64_t t_count, float eps2, float scale, int final_out, float4 *out, int64_t out_stride,
-                         const int *mass_flag, int generation, cudaStream_t st) {
+                         const int *mass_flag, int generation, int *step_ctr, cudaStream_t st, bool pdl) {
     switch (geo.IP) {
         case 3:
             return launch_force_variant<3, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
-                                                      final_out, out, out_stride, mass_flag, generation, st);
+                                                      final_out, out, out_stride, mass_flag, generation, step_ctr, st, pdl);
         case 2:
             return launch_force_variant<2, 512, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
-                                                     final_out, out, out_stride, mass_flag, generation, st);
+                                                     final_out, out, out_stride, mass_flag, generation, step_ctr, st, pdl);
         default:
-            return launch_force_variant<1, 256, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
-                                                     final_out, out, out_stride, mass_flag, generation, st);
+            return launch_force_variant<1, 128, POT>(geo, pos_mass, packed, t_begin, t_count, eps2, scale,
+                                                     final_out, out, out_stride, mass_flag, generation, step_ctr, st, pdl);
     }
 }
 
@@ -199,6 +226,14 @@ cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const floa
 struct FusedStep {
     StepSrc src;
     int deferred_splits = 0;
+    // two-kernel step loop of colatus_run: the staged array was written by the previous tail/head kernel (no staging
+    // launch here), one equal-mass generation stamp serves the whole run, and the force kernel hands the step
+    // counter over (force_kernels.cuh)
+    bool skip_stage = false;
+    int fixed_generation = 0;
+    int *step_ctr = nullptr;
+    bool pdl = false;          // launch the force kernel as a programmatic dependent of its predecessor
+    Geometry geo;              // out: the geometry used (n_pad for the tail/head kernel's grid)
 };
 
 int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2, float4 *out,
@@ -214,16 +249,26 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     // equal-mass detection: a fresh generation per force evaluation; a body whose mass differs from body 0's
     // stamps it into the flag, the force kernel compares (force_kernels.cuh)
     int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
-    g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
-    const int generation = g.generation;
-    if (fused)
-        drift_stage_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(g.pos, g.vel, n, geo.n_pad, packed,
-                                                                                mass_flag, generation, fused->src);
-    else
-        stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed,
-                                                                                  mass_flag, generation);
-    CUDA_TRY(cudaGetLastError());
-    g.launches++;
+    int generation;
+    if (fused && fused->fixed_generation) {
+        generation = fused->fixed_generation;
+    } else {
+        g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
+        generation = g.generation;
+    }
+    if (fused) fused->geo = geo;
+    if (fused && fused->skip_stage) {
+        // staged by the caller's tail/head kernel
+    } else {
+        if (fused)
+            drift_stage_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(g.pos, g.vel, n, geo.n_pad, packed,
+                                                                                    mass_flag, generation, fused->src);
+        else
+            stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed,
+                                                                                      mass_flag, generation);
+        CUDA_TRY(cudaGetLastError());
+        g.launches++;
+    }
 
     const bool single = geo.splits == 1;
     float4 *fout = single ? out : partials;
@@ -241,10 +286,12 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         e1 = g.ev_pool[g.ev_used++];
         CUDA_TRY(cudaEventRecord(e0, st));
     }
+    int *step_ctr = fused ? fused->step_ctr : nullptr;
     cudaError_t e = potential ? launch_force<true>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single, fout,
-                                                   t_count, mass_flag, generation, st)
+                                                   t_count, mass_flag, generation, step_ctr, st, fused && fused->pdl)
                               : launch_force<false>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single,
-                                                    fout, t_count, mass_flag, generation, st);
+                                                    fout, t_count, mass_flag, generation, step_ctr, st,
+                                                    fused && fused->pdl);
     CUDA_TRY(e);
     g.launches++;
     if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
@@ -376,7 +423,7 @@ int enqueue_step_scalar(double d1, double cv, double ck, double d2, float tag) {
     return enqueue_force_kick_drift(cv, ck, d2, tag);
 }
 
-void invalidate_graph() { g.graph_valid = false; }
+void invalidate_graph() { g.graph_valid = false; }   // both graphs are rebuilt at the next colatus_run
 
 // One step with the coefficients of table row ctr[0] (integrate_kernels.cuh "table-driven variants"):
 // the same launches as colatus_step (fused when possible), with step-independent arguments, on stream `st`.
@@ -402,6 +449,56 @@ int enqueue_step_table(cudaStream_t st) {
         kick_drift_table_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, table, ctr,
                                                                nullptr, nullptr, 0);
     }
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
+// ---- two-kernel step loop of colatus_run (whole range, no external terms; integrate_kernels.cuh) --------------
+// head: the first half drift + staging of the run's first step (row ctr[0] of the table);
+// step: force kernel (+ step-counter hand-over) and the tail/head kernel.  `generation` is one equal-mass stamp
+// for the whole run (a captured graph keeps replaying the same value).
+int enqueue_run_head(cudaStream_t st, int generation) {
+    const Workspace w = workspace_layout(g.n);
+    const Geometry geo = choose_geometry(g.n, g.n);
+    const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
+    int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
+    float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
+    int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
+    StepSrc src{table, ctr, 0.f, 0.f, 0.f, 0.f, 0.f, 0};
+    drift_stage_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(g.pos, g.vel, g.n, geo.n_pad, packed, mass_flag,
+                                                                            generation, src);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
+int enqueue_step_two_kernels(cudaStream_t st, int generation) {
+    const Workspace w = workspace_layout(g.n);
+    const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
+    int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
+    FusedStep f;
+    f.skip_stage = true;
+    f.fixed_generation = generation;
+    f.step_ctr = ctr;
+    f.pdl = true;
+    int rc = run_forces(g.pos, g.n, 0, g.n, g.eps2, g.acc, false, st, &f);
+    if (rc) return rc;
+    const unsigned blocks = (unsigned)((f.geo.n_pad + 255) / 256);
+    const int32_t *slot = reinterpret_cast<const int32_t *>(g.ws + w.trace_slot);
+    const float4 *partials = reinterpret_cast<const float4 *>(g.ws + w.partials);
+    float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
+    int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
+    cudaError_t e;
+    if (g.trace_k > 0)
+        e = launch_ex(step_tail_head_kernel<true>, dim3(blocks), dim3(256), 0, st, true, g.pos, g.vel, g.acc, partials,
+                      g.n, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, slot, g.ring, g.trace_k, packed,
+                      mass_flag, generation);
+    else
+        e = launch_ex(step_tail_head_kernel<false>, dim3(blocks), dim3(256), 0, st, true, g.pos, g.vel, g.acc, partials,
+                      g.n, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, (const int32_t *)nullptr,
+                      (float4 *)nullptr, 0, packed, mass_flag, generation);
+    CUDA_TRY(e);
     CUDA_TRY(cudaGetLastError());
     g.launches++;
     return COLATUS_OK;
@@ -467,6 +564,10 @@ int colatus_init(const colatus_config *cfg) {
 void colatus_shutdown(void) {
     if (g.graph_exec) cudaGraphExecDestroy(g.graph_exec);
     if (g.graph) cudaGraphDestroy(g.graph);
+    if (g.graph_exec_k) cudaGraphExecDestroy(g.graph_exec_k);
+    if (g.graph_k) cudaGraphDestroy(g.graph_k);
+    g.graph_exec_k = nullptr;
+    g.graph_k = nullptr;
     if (g.run_ev_in) cudaEventDestroy(g.run_ev_in);
     if (g.run_ev_out) cudaEventDestroy(g.run_ev_out);
     if (g.run_stream) cudaStreamDestroy(g.run_stream);
@@ -686,7 +787,12 @@ static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t
         q.d2 = (float)k[3];
         q.tag = (float)tag;
         q.ring_row = g.trace_k > 0 ? (int)((g.step + s) % g.trace_cap) : 0;
-        q.pad0 = q.pad1 = 0.f;
+        q.d1_next = 0.f;
+        q.has_next = 0;
+        if (s > 0) {                                         // two-kernel loop: the tail of step s-1 does this step's head
+            coef[(size_t)s - 1].d1_next = q.d1;
+            coef[(size_t)s - 1].has_next = 1;
+        }
     }
 
     if (!g.run_stream) {
@@ -702,24 +808,45 @@ static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t
     const bool profile_was = g.profile;
     g.profile = false;                                      // no event brackets inside a graph
     int rc = COLATUS_OK;
+    // whole-range runs without external terms take the two-kernel loop (force + tail/head per step, one head
+    // kernel per run); otherwise a step is drift / force (+ reduce, external terms) / kick-drift
+    const bool two = can_fuse_step();
+    int run_generation = 0;
+    if (two && !use_graph) {
+        g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
+        run_generation = g.generation;
+    }
     if (use_graph && !g.graph_valid) {
         if (g.graph_exec) cudaGraphExecDestroy(g.graph_exec);
         if (g.graph) cudaGraphDestroy(g.graph);
-        g.graph_exec = nullptr;
-        g.graph = nullptr;
-        cudaError_t e = cudaStreamBeginCapture(g.run_stream, cudaStreamCaptureModeThreadLocal);
-        if (e == cudaSuccess) {
-            const int64_t launches0 = g.launches;
-            rc = enqueue_step_table(g.run_stream);
-            g.graph_launches = g.launches - launches0;      // kernels per replay
-            g.launches = launches0;                         // captured, not launched
-            e = cudaStreamEndCapture(g.run_stream, &g.graph);
-            if (rc == COLATUS_OK && e == cudaSuccess) e = cudaGraphInstantiate(&g.graph_exec, g.graph, 0);
+        if (g.graph_exec_k) cudaGraphExecDestroy(g.graph_exec_k);
+        if (g.graph_k) cudaGraphDestroy(g.graph_k);
+        g.graph_exec = g.graph_exec_k = nullptr;
+        g.graph = g.graph_k = nullptr;
+        g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
+        g.graph_generation = g.generation;                  // the captured kernels keep stamping / comparing this value
+        // a one-step graph, and for the two-kernel loop also a graph of GRAPH_STEPS consecutive steps (the step
+        // index lives on the device, so every step's nodes are identical): replaying several steps at once
+        // removes the gap between graph launches, which at N = 4096 is a quarter of a step
+        for (int pass = 0; pass < (two ? 2 : 1) && rc == COLATUS_OK; ++pass) {
+            cudaGraph_t *gr = pass ? &g.graph_k : &g.graph;
+            cudaGraphExec_t *ge = pass ? &g.graph_exec_k : &g.graph_exec;
+            cudaError_t e = cudaStreamBeginCapture(g.run_stream, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+                const int64_t launches0 = g.launches;
+                for (int k = 0; k < (pass ? GRAPH_STEPS : 1) && rc == COLATUS_OK; ++k)
+                    rc = two ? enqueue_step_two_kernels(g.run_stream, g.graph_generation) : enqueue_step_table(g.run_stream);
+                if (!pass) g.graph_launches = g.launches - launches0;      // kernels per step
+                g.launches = launches0;                                    // captured, not launched
+                e = cudaStreamEndCapture(g.run_stream, gr);
+                if (rc == COLATUS_OK && e == cudaSuccess) e = cudaGraphInstantiate(ge, *gr, 0);
+            }
+            if (rc == COLATUS_OK && e != cudaSuccess)
+                rc = fail(COLATUS_CUDA_ERROR, "graph capture failed: %s", cudaGetErrorString(e));
         }
-        if (rc == COLATUS_OK && e != cudaSuccess)
-            rc = fail(COLATUS_CUDA_ERROR, "graph capture failed: %s", cudaGetErrorString(e));
         g.graph_valid = rc == COLATUS_OK;
     }
+    if (use_graph) run_generation = g.graph_generation;
     StepCoef *table = reinterpret_cast<StepCoef *>(g.ws + w.step_table);
     int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
     for (int64_t s0 = 0; rc == COLATUS_OK && s0 < n_steps; s0 += RUN_CHUNK) {
@@ -731,15 +858,20 @@ static int run_steps(const colatus_cosmo *c, double a_start, double tau, int64_t
             rc = fail(COLATUS_CUDA_ERROR, "table upload failed: %s", cudaGetErrorString(e));
             break;
         }
-        for (int64_t s = 0; s < m && rc == COLATUS_OK; ++s) {
+        if (two && s0 == 0) rc = enqueue_run_head(g.run_stream, run_generation);   // later heads ride in the tails
+        for (int64_t s = 0; s < m && rc == COLATUS_OK;) {
+            int64_t done = 1;
             if (use_graph) {
-                e = cudaGraphLaunch(g.graph_exec, g.run_stream);
+                const bool multi = g.graph_exec_k && m - s >= GRAPH_STEPS;
+                if (multi) done = GRAPH_STEPS;
+                e = cudaGraphLaunch(multi ? g.graph_exec_k : g.graph_exec, g.run_stream);
                 if (e != cudaSuccess) rc = fail(COLATUS_CUDA_ERROR, "cudaGraphLaunch failed: %s", cudaGetErrorString(e));
-                g.launches += g.graph_launches;
+                g.launches += g.graph_launches * done;
             } else {
-                rc = enqueue_step_table(g.run_stream);
+                rc = two ? enqueue_step_two_kernels(g.run_stream, run_generation) : enqueue_step_table(g.run_stream);
             }
-            if (rc == COLATUS_OK) g.step++;
+            if (rc == COLATUS_OK) g.step += done;
+            s += done;
         }
     }
     g.profile = profile_was;
@@ -962,7 +1094,7 @@ int colatus_set_option(const char *name, int64_t value) {
         if (value != 0 && value != 2 && value != 4 && value != 6) return fail(COLATUS_INVALID_ARG, "must be 0,2,4,6");
         g.force_I = (int)value;
     } else if (!strcmp(name, "source_splits")) {
-        if (value < 0 || value > MAX_SPLITS) return fail(COLATUS_INVALID_ARG, "must be in [0, %d]", MAX_SPLITS);
+        if (value < 0 || value > MAX_SPLITS) return fail(COLATUS_INVALID_ARG, "must be in [0, %d]", MAX_SPLITS);   // capped per n
         g.force_splits = (int)value;
     } else {
         return fail(COLATUS_INVALID_ARG, "unknown option %s", name);

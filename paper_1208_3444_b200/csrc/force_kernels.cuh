@@ -94,6 +94,13 @@ __device__ __forceinline__ void bulk_copy_g2s(void *dst_smem, const void *src_gm
                  : "memory");
 }
 
+// ---- programmatic dependent launch (the two-kernel step loop of colatus_run chains force and tail/head kernels
+// with it): `wait` blocks until every kernel this launch depends on has finished and its writes are visible (a
+// no-op for an ordinary launch); `launch_dependents` lets the next kernel's CTAs be scheduled early, where they
+// sit in their own `wait` -- only launch latency and prologues overlap, never data accesses.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
 // ---- staging: padding of the source array, equal-mass detection -------------------------------------
 // staged[j] = pos_mass[j] for j < n, (FAR, FAR, FAR, 0) for n <= j < n_pad.  A padding source has mass 0
 // and sits 1e18 away: it contributes exactly 0 to F in the general loop (w = rinv^3 * 0) and in the
@@ -225,7 +232,8 @@ template <int IP, int TJ, int NST, bool POT, int MINB>
 __global__ void __launch_bounds__(FORCE_THREADS, MINB)
 force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ staged, int64_t t_begin,
              int64_t t_count, int tiles_per_split, float eps2, float scale, int final_out,
-             float4 *__restrict__ out, int64_t out_stride, const int *__restrict__ mass_flag, int generation) {
+             float4 *__restrict__ out, int64_t out_stride, const int *__restrict__ mass_flag, int generation,
+             int *__restrict__ step_ctr) {
     constexpr int TILE_BYTES = TJ * 16;
     constexpr int NC = POT ? 4 : 3;                                                  // components per target
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -246,6 +254,10 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
         mbar_fence_init();
     }
     __syncthreads();
+    griddep_wait();                 // nothing above touches global memory; everything below may read the predecessor's output
+    griddep_launch_dependents();
+    // two-kernel step loop (integrate_kernels.cuh): hand the step index from the previous tail to the next one
+    if (step_ctr && tid == 0 && blockIdx.x == 0 && blockIdx.y == 0) step_ctr[1] = step_ctr[0];
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < NST; ++s)
@@ -307,25 +319,28 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
     }
 }
 
-constexpr int REDUCE_MAX_SPLITS = 16;   // upper bound on source splits (partials held in registers below)
+constexpr int REDUCE_MAX_SPLITS = 64;   // upper bound on source splits (small problems; large ones use <= 16)
+constexpr int REDUCE_CHUNK = 16;        // partials loaded together (held in registers below)
 
-// Sum of the `splits` partials of target t in split order 0, 1, 2, ...: all loads first (independent, so
-// their latencies overlap), then the adds in fixed order.
+// Sum of the `splits` partials of target t in split order 0, 1, 2, ...: 16 loads at a time (independent, so
+// their latencies overlap), then the adds in fixed order -- the result does not depend on the chunking.
 __device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partial, int64_t stride, int splits,
                                                int64_t t) {
-    constexpr int MAXS = REDUCE_MAX_SPLITS;
-    float4 q[MAXS];
+    float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k0 = 0; k0 < splits; k0 += REDUCE_CHUNK) {
+        float4 q[REDUCE_CHUNK];
 #pragma unroll
-    for (int k = 0; k < MAXS; ++k)
-        q[k] = k < splits ? partial[(size_t)k * stride + t] : make_float4(0.f, 0.f, 0.f, 0.f);
-    float4 s = q[0];
+        for (int k = 0; k < REDUCE_CHUNK; ++k)
+            q[k] = k0 + k < splits ? partial[(size_t)(k0 + k) * stride + t] : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (k0 == 0) s = q[0];
 #pragma unroll
-    for (int k = 1; k < MAXS; ++k) {
-        if (k < splits) {
-            s.x += q[k].x;
-            s.y += q[k].y;
-            s.z += q[k].z;
-            s.w += q[k].w;
+        for (int k = 0; k < REDUCE_CHUNK; ++k) {
+            if (k0 + k < splits && (k0 + k) > 0) {
+                s.x += q[k].x;
+                s.y += q[k].y;
+                s.z += q[k].z;
+                s.w += q[k].w;
+            }
         }
     }
     return s;

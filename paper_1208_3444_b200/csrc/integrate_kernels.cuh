@@ -14,6 +14,13 @@
 
 namespace colatus {
 
+// The drift kernels update x, y, z only and never store .w, so that the mass a neighbouring thread may be reading
+// (body 0's, for the equal-mass detection) is not written concurrently.
+__device__ __forceinline__ void store_xyz(float4 *dst, const float4 &p) {
+    *reinterpret_cast<float2 *>(dst) = make_float2(p.x, p.y);
+    reinterpret_cast<float *>(dst)[2] = p.z;
+}
+
 // eq. (3): x += d v   (mass in .w untouched)
 __global__ void __launch_bounds__(256) drift_kernel(float4 *__restrict__ pos_mass, const float4 *__restrict__ vel,
                                                     int64_t begin, int64_t count, float d) {
@@ -63,7 +70,8 @@ kick_drift_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, const
 struct StepCoef {
     float d1, cv, ck, d2, tag;
     int ring_row;       // (step % capacity) of this step's tracer row
-    float pad0, pad1;   // 32 B per row
+    float d1_next;      // first half-drift coefficient of the step after this one (two-kernel loop below)
+    int has_next;       // 0 for the last step of a colatus_run call; 32 B per row
 };
 
 __global__ void __launch_bounds__(256)
@@ -136,13 +144,13 @@ drift_stage_kernel(float4 *__restrict__ pos_mass, const float4 *__restrict__ vel
     }
     if (j >= n_pad) return;
     if (j < n) {
-        const float m0 = pos_mass[0].w;          // body 0's mass: its .w is never changed by the drift
+        const float m0 = pos_mass[0].w;          // body 0's mass: no thread of this kernel stores a .w (store_xyz)
         float4 p = pos_mass[j];
         const float4 v = vel[j];
         p.x = fmaf(d, v.x, p.x);
         p.y = fmaf(d, v.y, p.y);
         p.z = fmaf(d, v.z, p.z);
-        pos_mass[j] = p;
+        store_xyz(pos_mass + j, p);
         staged[j] = p;
         if (p.w != m0) mass_flag[0] = generation;
     } else {
@@ -183,6 +191,75 @@ reduce_kick_drift_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel
         const int32_t t = trace_slot[i];
         if (t >= 0) ring[(size_t)ring_row * trace_k + t] = make_float4(v.x, v.y, v.z, tag);
     }
+}
+
+// ---- two-kernel step loop of colatus_run ------------------------------------------------------------------
+// Inside a run the tail of step s (partial sums, kick, drift, tracer record) and the head of step s+1 (first
+// half drift, staging, equal-mass detection) are consecutive elementwise passes over the same bodies, so they
+// share a kernel: a step is then TWO launches, force_kernel + step_tail_head_kernel (the very first head of a
+// run is one drift_stage_kernel).  Statement for statement the arithmetic is that of reduce_kick_drift_kernel
+// followed by drift_stage_kernel -- two separately rounded drifts, not one merged one -- so the bits equal
+// those of colatus_step.  Row ctr[1] of the table holds the step's coefficients plus d1 of the next step;
+// has_next = 0 on the last step of the run leaves x^{n+1} in place.  splits = 0: acc already holds G * sum.
+// The grid covers n_pad (the padding of the staged array is rewritten with far-away massless bodies).
+template <bool TRACE>
+__global__ void __launch_bounds__(256)
+step_tail_head_kernel(float4 *__restrict__ pos_mass, float4 *__restrict__ vel, float4 *__restrict__ acc,
+                      const float4 *__restrict__ partial, int64_t stride, int splits, int64_t n, int64_t n_pad,
+                      float G, const StepCoef *__restrict__ table, int *__restrict__ ctr,
+                      const int32_t *__restrict__ trace_slot, float4 *__restrict__ ring, int trace_k,
+                      float4 *__restrict__ staged, int *__restrict__ mass_flag, int generation) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // Launched as a programmatic dependent of the force kernel: everything the force kernel does not write --
+    // positions, velocities, the tracer map -- is loaded BEFORE the wait, so these loads overlap the end of the
+    // force kernel; only the step counter, the partial sums and acc wait for it.
+    float4 p = make_float4(0.f, 0.f, 0.f, 0.f), v = p;
+    float m0 = 0.f;
+    int32_t tslot = -1;
+    if (i < n) {
+        p = pos_mass[i];
+        v = vel[i];
+        m0 = pos_mass[0].w;                       // no thread of this kernel stores a .w (store_xyz)
+        if (TRACE) tslot = trace_slot[i];
+    }
+    griddep_wait();
+    griddep_launch_dependents();
+    const int s = ctr[1];                        // set by the force kernel of this step (ctr[1] = ctr[0])
+    if (i == 0) ctr[0] = s + 1;
+    if (i >= n_pad) return;
+    float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (i < n) {                                 // issued together with the counter load: independent of it
+        if (splits > 0) {
+            const float4 s4 = sum_partials(partial, stride, splits, i);
+            f = make_float4(s4.x * G, s4.y * G, s4.z * G, 0.f);
+            acc[i] = f;                           // the caller's acc buffer still receives F
+        } else {
+            f = acc[i];
+        }
+    }
+    const StepCoef c = table[s];
+    if (i >= n) {
+        if (c.has_next) staged[i] = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+        return;
+    }
+    v.x = fmaf(c.ck, f.x, c.cv * v.x);
+    v.y = fmaf(c.ck, f.y, c.cv * v.y);
+    v.z = fmaf(c.ck, f.z, c.cv * v.z);
+    p.x = fmaf(c.d2, v.x, p.x);
+    p.y = fmaf(c.d2, v.y, p.y);
+    p.z = fmaf(c.d2, v.z, p.z);
+    vel[i] = v;
+    if (TRACE) {
+        if (tslot >= 0) ring[(size_t)c.ring_row * trace_k + tslot] = make_float4(v.x, v.y, v.z, c.tag);
+    }
+    if (c.has_next) {                             // head of the next step: eq. (3) and the staged copy
+        p.x = fmaf(c.d1_next, v.x, p.x);
+        p.y = fmaf(c.d1_next, v.y, p.y);
+        p.z = fmaf(c.d1_next, v.z, p.z);
+        staged[i] = p;
+        if (p.w != m0) mass_flag[0] = generation;
+    }
+    store_xyz(pos_mass + i, p);
 }
 
 // External terms added to the force of eq. (1) for the target range (acc indexed from 0):

@@ -120,17 +120,24 @@ def test_forces_at_the_smallest_accepted_eps2(session, equal_mass):
     assert e.value.code == B.INVALID_ARG
 
 
-@pytest.mark.parametrize("splits", [1, 2, 3, 5, 16])
-def test_forces_source_splits(session, splits):
+@pytest.mark.parametrize("splits,variant", [(1, 0), (2, 0), (3, 0), (5, 0), (16, 0), (33, 0), (37, 2), (64, 2)])
+def test_forces_source_splits(session, splits, variant):
+    """Forced source splits (up to 64 below 65536 bodies: the partial sums are added 16 at a time in fixed
+    order), with the automatic variant and with the 2-targets-per-thread small-problem variant."""
     cfg, pm, _ = inputs.make_config(3, n_override=20000)
     B.colatus_set_option("source_splits", splits)
+    B.colatus_set_option("targets_per_thread", variant)
     try:
-        out = session.forces(pm, cfg.eps2).cpu().numpy()
+        geo = B.colatus_force_geometry(cfg.n)
+        out = session.forces(pm, cfg.eps2, potential=True).cpu().numpy()
     finally:
         B.colatus_set_option("source_splits", 0)
-    ref = oracle.forces(pm, cfg.eps2, 1.0)
+        B.colatus_set_option("targets_per_thread", 0)
+    assert geo["source_splits"] == splits
+    ref, phi = oracle.forces(pm, cfg.eps2, 1.0, potential=True)
     med, mx = force_errors(out[:, :3], ref)
     assert med <= MEDIAN_TOL and mx <= MAX_TOL, (splits, med, mx)
+    assert np.allclose(out[:, 3], phi, rtol=2e-5, atol=0)
 
 
 def test_forces_range_matches_full(session):

@@ -188,8 +188,9 @@ def test_trace_ring_wraps():
 
 
 def test_target_range_stepping_matches_full():
-    """Two half ranges stepped one after the other on shared arrays reproduce the full step bit for bit
-    (the single-GPU emulation of the target-sharded multi-GPU step)."""
+    """Two half ranges stepped one after the other on shared arrays reproduce the full step up to the summation
+    order (the source split is chosen per target count, reading G14: FP32 sums differ at the 1e-6 level between
+    tilings) -- the single-GPU emulation of the target-sharded multi-GPU step."""
     import torch
     cfg, pm, vel = inputs.make_config(1)
     with _session(cfg.G, cfg.n) as s:
@@ -215,7 +216,8 @@ def test_target_range_stepping_matches_full():
         pos, v = s.download()
         pos[:h] = new_pos[0].cpu().numpy()
         pos[h:] = new_pos[1].cpu().numpy()
-    assert np.allclose(pos, full_pos, rtol=0, atol=1e-7) and np.allclose(v, full_vel, rtol=2e-6, atol=1e-7)
+    v_rms = float(np.sqrt((full_vel[:, :3].astype(np.float64) ** 2).sum(1).mean()))
+    assert np.abs(pos - full_pos).max() <= 1e-7 and np.abs(v - full_vel).max() <= 2e-6 * v_rms
 
 
 @pytest.mark.parametrize("index,n_override", [(1, None), (3, 100), (3, 20000)])
