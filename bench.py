@@ -40,8 +40,8 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-kernel launch from the `ncu --set full` capture
 # summarised in profiles/: valid only for the (n, source splits) it was captured at -- reported as null otherwise.
-FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 130877184, "n": 1 << 20, "splits": 8,
-                             "profile": "profiles/r01_force_kernel_ncu_full.txt"}
+FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8,
+                             "profile": "profiles/r02_force_kernel_ncu_full.txt"}
 # executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
 # (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention
 EXECUTED_FLOP_GENERAL, EXECUTED_FLOP_EQUAL_MASS = 19.0, 18.0

@@ -27,6 +27,12 @@
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - One implicit process-wide context (one GPU per process).  Calls are not
  *     thread-safe; serialise them.
+ *   - ONE workspace serves every entry point (staged sources, partial sums, the equal-mass flag,
+ *     host-buffer staging, step table): work enqueued through this library must be stream-ordered
+ *     as a whole.  Serialising the host calls is not enough -- two evaluations on different
+ *     streams, or a colatus_forces* / colatus_splat call on a stream other than the resident one
+ *     while resident work (colatus_step, colatus_run, colatus_diagnostics) is still in flight, race
+ *     on the device.  Use one stream, or order the streams with events before each call.
  *   - Every function returning int returns COLATUS_OK (0) or a negative
  *     colatus_status; on error no output is written and colatus_last_error()
  *     describes the failure.  No exception or abort crosses the ABI.
@@ -145,11 +151,16 @@ int colatus_step_coeffs(double d1, double cv, double ck, double d2);
  *   a_mid = a(t_n + tau/2), H_mid = H(a_mid)  (reading G3),  then a(t_n + tau);
  * c == NULL means a static background (a = 1, H = 0; a_start ignored).  The per-step
  * coefficients go to a device table (in the workspace, 1024 steps per upload) and a device
- * counter selects the row, so every step launches the same kernels with the same arguments:
- * with use_graph != 0 one captured CUDA graph of the step (drift + staging, force, partial-sum
- * reduction + kick + drift + tracer record) is replayed per step -- this is what makes the launch-bound
- * small-N loops (configs 1-3) fast; with use_graph == 0 the same kernels are launched one by
- * one (for comparison).  Results are bitwise identical to n_steps calls of colatus_step.
+ * counter selects the row, so every step launches the same kernels with the same arguments.
+ * Whole-range runs without external terms take TWO launches per step: the force kernel, and one
+ * tail/head kernel (partial-sum reduction + kick + drift + tracer record of step s, then the first
+ * half drift + source staging of step s+1 -- two separately rounded drifts, as in colatus_step),
+ * chained by programmatic dependent launch; only the first head of a run is a launch of its own.
+ * With use_graph != 0 captured CUDA graphs of 8 steps (and of 1 step for the remainder) are
+ * replayed -- this is what makes the launch-bound small-N loops (configs 1-3) fast; with
+ * use_graph == 0 the same kernels are launched one by one.  Target sub-ranges and runs with
+ * external terms take drift / force (+ reduction, external terms) / kick-drift launches instead.
+ * Results are bitwise identical to n_steps calls of colatus_step.
  * The loop runs on a stream owned by the library, ordered after everything already enqueued
  * on the resident stream and before everything enqueued on it later.  *a_end (may be NULL)
  * receives a(t_0 + n_steps tau).  Nothing is enqueued if any step's coefficients are invalid

@@ -256,8 +256,6 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
     __syncthreads();
     griddep_wait();                 // nothing above touches global memory; everything below may read the predecessor's output
     griddep_launch_dependents();
-    // two-kernel step loop (integrate_kernels.cuh): hand the step index from the previous tail to the next one
-    if (step_ctr && tid == 0 && blockIdx.x == 0 && blockIdx.y == 0) step_ctr[1] = step_ctr[0];
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < NST; ++s)
@@ -286,6 +284,11 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
     const u64 eps2_2 = pack2(eps2, eps2);
 #pragma unroll
     for (int c = 0; c < IP * NC; ++c) acc2[c * FORCE_THREADS + tid] = 0ull;   // private to this thread
+
+    // two-kernel step loop (integrate_kernels.cuh): hand the step index from the previous tail to the next one.  Done
+    // by the last thread of one CTA once its own loads are in flight, so the round trip hides behind the first
+    // tile's arrival instead of delaying the producer thread's bulk copies.
+    if (step_ctr && tid == FORCE_THREADS - 1 && blockIdx.x == 0 && blockIdx.y == 0) step_ctr[1] = step_ctr[0];
 
     // equal masses <=> no body stamped this launch's generation (stage_sources_kernel); uniform over the grid
     const bool eqm = __ldg(mass_flag) != generation;
