@@ -141,7 +141,8 @@ Workspace workspace_layout(int64_t n_max) {
 
 // Pick the kernel variant (target pairs per thread, tile) and the source split by a cost model fitted to
 // a sweep of every (variant, split) at N = 4096 ... 262144 on the B200 (DESIGN.md 6.3 "Launch geometry";
-// rms error 2 %, picks within 0.7 % of the best measured geometry at every size):
+// tool: paper_1208_3444_b200/tune_geometry.py, data: profiles/r02_geometry_sweep.md -- picks within 0.6 % of the best
+// measured geometry with <= 16 splits at every size but N = 8192 (+5 %)):
 //   time ~ a_IP * IP * S * (per_sm + 0.1) + per_sm * c0
 // S = padded sources per split, per_sm = ceil(CTAs / SMs) (an SM works through its CTAs two at a time,
 // work-conserving, so what counts is CTAs per SM, not waves of resident slots), a_IP = time per source and
@@ -149,7 +150,10 @@ Workspace workspace_layout(int64_t n_max) {
 // (n, t_count, SM count): the geometry, and with it the summation order, is reproducible.
 Geometry choose_geometry(int64_t n, int64_t t_count) {
     static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 128}};   // (target pairs per thread, tile)
-    static const double a_us[4] = {0.0, 0.0295, 0.0287, 0.0274};        // per source, per target pair
+    // per source, per target pair.  a_us[2] was 0.0287 in round 1; the round-2 sweep (profiles/r02_geometry_sweep.md)
+    // shows the 4-targets-per-thread variant level with the 6-target one for equal masses, and 0.0283 moves
+    // N = 131072 from 86 x 12 (+3.4 % over the best measured) to 128 x 16 (+0.2 %) with no other pick changed
+    static const double a_us[4] = {0.0, 0.0295, 0.0283, 0.0274};
     const double c0_us = 0.77, ramp = 0.096;
     Geometry best;
     double best_cost = -1.0;

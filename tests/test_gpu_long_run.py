@@ -25,9 +25,11 @@ The 64-tracer speed percentiles of SURVEY G20 ("median and 90th percentile withi
 relative bar: between the two ORACLE runs they differ by up to 17 % (median) and 21 % (p90) -- 64 samples of a
 chaotic flow (tests/test_long_run_calibration.py asserts these numbers from the committed JSON).  They are
 tested in the units in which their scatter is known instead: the position of the tracers' median / p90 inside the
-oracle's all-particle speed distribution has a binomial standard error sqrt(q (1 - q) / 64) = 6.25 / 3.75
-percentile points, and the GPU run must sit within 4 sigma (25 / 15 points) of where run A's tracers sit.  While
-the flow is laminar (step <= 50) every tracer's speed is compared one by one.
+oracle's all-particle speed distribution has a binomial standard error sigma = sqrt(q (1 - q) / 64) = 6.25 / 3.75
+percentile points PER RUN; the GPU run and run A are two such draws, so their difference scatters with
+sqrt(2) sigma, and the GPU run must sit within 4 sqrt(2) sigma (35 / 21 points) of where run A's tracers sit
+(A and B differ by up to 10 points, 1.9 sqrt(2) sigma).  While the flow is laminar (step <= 50) every tracer's
+speed is compared one by one.
 """
 import importlib.util
 import json
@@ -118,12 +120,12 @@ def test_config2_full_size_1000_steps_statistics():
         ts_ref = np.array(r["tracer_speed"])
         if r["step"] <= 50:                                            # laminar: tracer by tracer
             assert np.abs(g["tracer_speed"] - ts_ref).max() <= 1e-3 * np.sqrt((ts_ref ** 2).mean()), r["step"]
-        else:                                                          # chaotic: within 4 binomial sigma of run A
+        else:                                                          # chaotic: two 64-sample draws, 4 sqrt(2) sigma
             for q, sigma_pts in ((50, 6.25), (90, 3.75)):
                 at_gpu = _parent_percentile(np.percentile(g["tracer_speed"], q), r)
                 at_ref = _parent_percentile(np.percentile(ts_ref, q), r)
                 worst[f"tracer_q{q}_points"] = max(worst.get(f"tracer_q{q}_points", 0.0), abs(at_gpu - at_ref))
-                assert abs(at_gpu - at_ref) <= 4.0 * sigma_pts, (r["step"], q, at_gpu, at_ref)
+                assert abs(at_gpu - at_ref) <= 4.0 * np.sqrt(2.0) * sigma_pts, (r["step"], q, at_gpu, at_ref)
     record_parity("1000-step config 2 at 32^3 vs golden oracle run", **worst)
 
     # the run is not trivial: the box collapses onto its centre (G7) and the kinetic energy grows several-fold

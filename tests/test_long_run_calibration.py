@@ -74,8 +74,9 @@ def test_one_ulp_sensitivity_at_full_size_is_what_the_docs_quote():
     tm = _self_differences(c2, lambda r: float(np.median(r["tracer_speed"])))
     tp = _self_differences(c2, lambda r: float(np.percentile(r["tracer_speed"], 90)))
     assert max(tm[s] for s in chaotic) > 0.15 and max(tp[s] for s in chaotic) > 0.20
-    # ... while, measured in percentile points of the all-particle distribution, A and B stay within 3 binomial
-    # sigma of each other (sigma = 6.25 points at the median, 3.75 at p90): the unit the GPU test uses
+    # ... while, measured in percentile points of the all-particle distribution, A and B stay within 3 sigma of each
+    # other, sigma = 6.25 points at the median, 3.75 at p90 per run (two runs differ with sqrt(2) sigma, so this is
+    # 2.1 sigma of the difference): the unit the GPU test uses, with 4 sqrt(2) sigma
     for ra, rb in zip(c2["A"]["checkpoints"], c2["B"]["checkpoints"]):
         for q, sigma in ((50, 6.25), (90, 3.75)):
             pa = np.interp(np.percentile(ra["tracer_speed"], q), ra["speed_q"], G.QUANTILES)
