@@ -71,6 +71,7 @@ SIGNATURES = {
     "colatus_profile_read": (c_int, [POINTER(c_double), POINTER(c_int64)]),
     "colatus_launch_count": (c_int64, []),
     "colatus_force_geometry": (c_int, [c_int64, c_int64, POINTER(c_int64)]),
+    "colatus_force_plan": (c_int, [c_int64, c_int64, c_int, POINTER(c_int64)]),
     "colatus_set_option": (c_int, [c_char_p, c_int64]),
     "colatus_last_error": (c_char_p, []),
     "colatus_hubble": (c_double, [POINTER(colatus_cosmo), c_double]),
@@ -300,6 +301,15 @@ def colatus_force_geometry(n, target_count=None):
     _check(lib().colatus_force_geometry(int(n), int(n if target_count is None else target_count), out))
     keys = ("targets_per_cta", "target_tiles", "source_splits", "sources_per_split", "ctas_per_sm", "sm_count",
             "targets_per_thread", "threads_per_cta")
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def colatus_force_plan(n, target_count=None, with_potential=False):
+    out = (c_int64 * 8)()
+    _check(lib().colatus_force_plan(int(n), int(n if target_count is None else target_count),
+                                    1 if with_potential else 0, out))
+    keys = ("symmetric", "blocks", "splits", "distances", "distances_per_launch", "launches", "padded_bodies",
+            "partial_rows")
     return dict(zip(keys, [int(v) for v in out]))
 
 

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcolatus.so")
 SOURCES = ["colatus_api.cu", "cosmo_host.cpp"]
-HEADERS = ["force_kernels.cuh", "integrate_kernels.cuh", "analysis_kernels.cuh", os.path.join("..", "..", "include", "colatus.h")]
+HEADERS = ["force_kernels.cuh", "force_sym_kernels.cuh", "integrate_kernels.cuh", "analysis_kernels.cuh", os.path.join("..", "..", "include", "colatus.h")]
 PROBE_LIB = os.path.join(HERE, "libcolatus_probe.so")
 PROBE_SOURCES = ["colatus_probe.cu"]
 PROBE_HEADERS = ["probe_kernels.cuh", "force_kernels.cuh", os.path.join("..", "..", "include", "colatus_probe.h")]

@@ -13,6 +13,7 @@
 
 #include "../../include/colatus.h"
 #include "force_kernels.cuh"
+#include "force_sym_kernels.cuh"
 #include "integrate_kernels.cuh"
 #include "analysis_kernels.cuh"
 
@@ -29,11 +30,24 @@ constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
 constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in colatus_run
 constexpr int GRAPH_STEPS = 8;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
 
+// symmetric (each pair once) force kernel, force_sym_kernels.cuh: whole-range evaluations of at least SYM_MIN_N bodies
+constexpr int SYM_IP = 3, SYM_TJ = 512;
+constexpr int64_t SYM_BT = (int64_t)FORCE_THREADS * 2 * SYM_IP;   // bodies per block = targets of one CTA
+constexpr int SYM_TPB = (int)(SYM_BT / SYM_TJ);                   // tiles per block
+constexpr int64_t SYM_MIN_N = 49152;
+constexpr int SYM_MAX_SPLITS = 16;
+constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch can always hold
+constexpr size_t SYM_ROWS_BUDGET = (size_t)8 << 30;               // bytes of partial rows before an evaluation is chunked
+
 struct Geometry {
     int IP = 0, TJ = 0;   // target pairs per thread, sources per tile
     int64_t tiles_t = 0;
     int splits = 0, tiles_per_split = 0;
     int64_t n_pad = 0;   // sources covered = splits * tiles_per_split * TJ
+    // symmetric kernel: nb blocks of SYM_BT bodies (n_pad = nb * SYM_BT, tiles_t = nb), H block distances,
+    // K of them per launch (K reaction rows + `splits` target-side rows in the workspace), `chunks` launches
+    bool sym = false;
+    int nb = 0, H = 0, K = 0, chunks = 0;
 };
 
 struct Workspace {     // byte offsets inside the caller's workspace
@@ -66,6 +80,8 @@ struct Context {
     int64_t launches = 0;
     // tuning overrides (0 = automatic)
     int force_I = 0, force_splits = 0;
+    int sym_rows = 0;     // cap on partial rows per launch of the symmetric kernel (0 = what the workspace holds)
+    int symmetric = 1;    // 0 = never, 1 = automatic (n >= SYM_MIN_N), 2 = whenever the evaluation allows it
     int init_epoch = 0;   // counts colatus_init calls
     int generation = 0;   // equal-mass detection stamp (never 0: the flag word starts at 0)
     // external terms: eq. (10) source and mean-density background (0 = off)
@@ -121,13 +137,33 @@ inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int max_splits(int64_t n) { return n <= SMALL_N ? MAX_SPLITS : MAX_SPLITS_LARGE; }
 
+// Bytes of partial-sum rows for n bodies: the source-split partials of force_kernel, and for n >= SYM_MIN_N the
+// rows of force_sym_kernel -- all of them ((splits + H) rows of n_pad bodies) while that stays within
+// SYM_ROWS_BUDGET, else the budget (the evaluation is then chunked over block distances), never fewer than
+// SYM_MAX_SPLITS + SYM_MIN_ROWS rows.  Non-decreasing in n, so a workspace sized for n_max serves every n <= n_max.
+inline int64_t sym_blocks(int64_t n) { return (n + SYM_BT - 1) / SYM_BT; }
+size_t partials_bytes(int64_t n) {
+    size_t bytes = (size_t)max_splits(n) * (size_t)n * 16;
+    const size_t row = (size_t)sym_blocks(n) * SYM_BT * 16;
+    if (bytes < (SYM_MAX_SPLITS + 2) * row) bytes = (SYM_MAX_SPLITS + 2) * row;   // tiny n with "symmetric" = 2
+    if (n >= SYM_MIN_N) {
+        const size_t H = (size_t)((sym_blocks(n) - 1) / 2);
+        size_t want = (SYM_MAX_SPLITS + H) * row;
+        if (want > SYM_ROWS_BUDGET) want = SYM_ROWS_BUDGET;
+        const size_t least = (size_t)(SYM_MAX_SPLITS + SYM_MIN_ROWS) * row;
+        if (want < least) want = least;
+        if (want > bytes) bytes = want;
+    }
+    return bytes;
+}
+
 Workspace workspace_layout(int64_t n_max) {
     Workspace w;
     const size_t n = (size_t)n_max;
     const size_t n_pad = round_up(n, (size_t)PAD_SOURCES) + (size_t)MAX_SPLITS * PAD_SOURCES;
     size_t off = 256;                        // [0, 256): mass_flag (zeroed by colatus_init)
     w.packed = off;      off += round_up(n_pad * 16, 256);
-    w.partials = off;    off += round_up((size_t)max_splits(n_max) * n * 16, 256);
+    w.partials = off;    off += round_up(partials_bytes(n_max), 256);
     w.scratch_acc = off; off += round_up(n * 16, 256);
     w.trace_slot = off;  off += round_up(n * 4, 256);
     w.diag = off;        off += round_up((size_t)(DIAG_BLOCKS_MAX + 2) * DIAG_Q * 8, 256);
@@ -148,7 +184,7 @@ Workspace workspace_layout(int64_t n_max) {
 // work-conserving, so what counts is CTAs per SM, not waves of resident slots), a_IP = time per source and
 // target pair of a CTA with the SM to itself, c0 = per-CTA prologue/epilogue.  Pure function of
 // (n, t_count, SM count): the geometry, and with it the summation order, is reproducible.
-Geometry choose_geometry(int64_t n, int64_t t_count) {
+Geometry choose_plain_geometry(int64_t n, int64_t t_count) {
     static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 128}};   // (target pairs per thread, tile)
     // per source, per target pair.  a_us[2] was 0.0287 in round 1; the round-2 sweep (profiles/r02_geometry_sweep.md)
     // shows the 4-targets-per-thread variant level with the 6-target one for equal masses, and 0.0283 moves
@@ -186,6 +222,78 @@ Geometry choose_geometry(int64_t n, int64_t t_count) {
         }
     }
     return best;
+}
+
+// Symmetric kernel (force_sym_kernels.cuh): whole-range evaluations without the potential, n >= SYM_MIN_N (or
+// forced by the "symmetric" option), automatic kernel variant.  nb blocks x S splits CTAs; S from the same kind
+// of cost model as above in units of one symmetric tile: (tiles per CTA) * (CTAs per SM + ramp) + CTAs per SM * c0.
+// K = block distances per launch = what the partial rows of workspace_layout(n) hold; a pure function of n.
+bool sym_eligible(int64_t n, int64_t t_count, bool potential) {
+    if (g.symmetric == 0 || potential || t_count != n || g.force_I != 0) return false;
+    return g.symmetric == 2 || n >= SYM_MIN_N;
+}
+
+Geometry choose_sym_geometry(int64_t n) {
+    Geometry geo;
+    geo.sym = true;
+    geo.IP = SYM_IP;
+    geo.TJ = SYM_TJ;
+    geo.nb = (int)sym_blocks(n);
+    geo.tiles_t = geo.nb;
+    geo.n_pad = (int64_t)geo.nb * SYM_BT;
+    geo.H = (geo.nb - 1) / 2;
+    int64_t rows_avail = (int64_t)(partials_bytes(n) / ((size_t)geo.n_pad * 16));
+    if (g.sym_rows >= 2 && g.sym_rows < rows_avail) rows_avail = g.sym_rows;   // "symmetric_rows": forces chunking
+    if (rows_avail < 2) {        // (forced on a tiny problem) no room for one target-side and one reaction row
+        geo.sym = false;
+        return geo;
+    }
+    const double plain_tiles = SYM_TPB * ((geo.nb & 1) ? 1.0 : 2.0) * 0.68;   // a one-directional tile costs ~0.68 symmetric ones
+    double best_cost = -1.0;
+    for (int s = 1; s <= SYM_MAX_SPLITS; ++s) {
+        if (g.force_splits && g.force_splits <= SYM_MAX_SPLITS && g.force_splits < rows_avail && s != g.force_splits)
+            continue;
+        if (s >= rows_avail) break;
+        int K = (int)(rows_avail - s);
+        if (K > geo.H) K = geo.H;
+        if (K < 1) K = 1;
+        const int chunks = geo.H == 0 ? 1 : (geo.H + K - 1) / K;
+        const double per_sm = (double)(((int64_t)geo.nb * s + g.sm_count - 1) / g.sm_count);
+        const double tiles = (plain_tiles + (double)SYM_TPB * geo.H) / s;
+        const double cost = tiles * (per_sm + 0.096) + chunks * per_sm * 0.04;
+        if (best_cost < 0.0 || cost < best_cost * 0.998) {
+            best_cost = cost;
+            geo.splits = s;
+            geo.K = K;
+            geo.chunks = chunks;
+        }
+    }
+    geo.tiles_per_split = (int)((SYM_TPB * (geo.H + 2) + geo.splits - 1) / geo.splits);
+    return geo;
+}
+
+Geometry choose_geometry(int64_t n, int64_t t_count, bool potential = false, bool single_launch = false) {
+    if (sym_eligible(n, t_count, potential)) {
+        const Geometry geo = choose_sym_geometry(n);
+        if (geo.sym && (!single_launch || geo.chunks == 1)) return geo;
+    }
+    return choose_plain_geometry(n, t_count);
+}
+
+cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
+                             float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
+                             cudaStream_t st, bool pdl) {
+    auto kern = force_sym_kernel<SYM_IP, SYM_TJ, NSTAGES, 2>;
+    const size_t smem = force_sym_smem_bytes<SYM_IP, SYM_TJ, NSTAGES>();
+    static int attr_epoch = 0;
+    if (attr_epoch != g.init_epoch) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_epoch = g.init_epoch;
+    }
+    dim3 grid((unsigned)geo.nb, (unsigned)geo.splits);
+    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, packed, geo.nb, geo.splits, k_begin, k_count,
+                     with_plain, eps2, partials, geo.n_pad, mass_flag, generation, step_ctr);
 }
 
 template <int IP, int TJ, bool POT>
@@ -230,6 +338,7 @@ cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const floa
 struct FusedStep {
     StepSrc src;
     int deferred_splits = 0;
+    int64_t deferred_stride = 0;   // bodies per partial row
     // two-kernel step loop of colatus_run: the staged array was written by the previous tail/head kernel (no staging
     // launch here), one equal-mass generation stamp serves the whole run, and the force kernel hands the step
     // counter over (force_kernels.cuh)
@@ -246,7 +355,7 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     if (w.total > g.ws_bytes)
         return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
                     (long long)n, w.total);
-    const Geometry geo = choose_geometry(n, t_count);
+    const Geometry geo = choose_geometry(n, t_count, potential, fused != nullptr);
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
     float4 *partials = reinterpret_cast<float4 *>(g.ws + w.partials);
 
@@ -274,9 +383,6 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         g.launches++;
     }
 
-    const bool single = geo.splits == 1;
-    float4 *fout = single ? out : partials;
-    const float scale = single ? (float)g.G : 1.0f;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (g.profile) {
         if (g.ev_used + 2 > g.ev_pool.size()) {
@@ -291,29 +397,63 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         CUDA_TRY(cudaEventRecord(e0, st));
     }
     int *step_ctr = fused ? fused->step_ctr : nullptr;
-    cudaError_t e = potential ? launch_force<true>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single, fout,
-                                                   t_count, mass_flag, generation, step_ctr, st, fused && fused->pdl)
-                              : launch_force<false>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single,
-                                                    fout, t_count, mass_flag, generation, step_ctr, st,
-                                                    fused && fused->pdl);
-    CUDA_TRY(e);
-    g.launches++;
-    if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
-
-    if (fused) {
-        fused->deferred_splits = single ? 0 : geo.splits;
-        return COLATUS_OK;                      // no external terms in fused steps (checked by the caller)
-    }
-    if (!single) {
-        const unsigned blocks = (unsigned)((t_count + 255) / 256);
-        if (potential)
-            reduce_partials_kernel<true><<<blocks, 256, 0, st>>>(partials, t_count, geo.splits, t_count, (float)g.G,
-                                                                 eps2, pos_mass, t_begin, out);
-        else
-            reduce_partials_kernel<false><<<blocks, 256, 0, st>>>(partials, t_count, geo.splits, t_count,
-                                                                  (float)g.G, eps2, pos_mass, t_begin, out);
-        CUDA_TRY(cudaGetLastError());
+    if (geo.sym) {
+        // every pair once (force_sym_kernels.cuh): one launch per chunk of block distances; its rows (target-side
+        // sums of the splits, then one reaction row per distance) are added in row order by the reduction -- here,
+        // or inside the caller's fused kick kernel (single-chunk geometries only)
+        const unsigned blocks = (unsigned)((n + 255) / 256);
+        for (int c = 0; c < geo.chunks; ++c) {
+            const int k_begin = 1 + c * geo.K;
+            const int k_count = geo.H - c * geo.K < geo.K ? geo.H - c * geo.K : geo.K;
+            CUDA_TRY(launch_force_sym(geo, packed, k_begin, k_count, c == 0, eps2, partials, mass_flag, generation,
+                                      c == 0 ? step_ctr : nullptr, st, fused && fused->pdl));
+            g.launches++;
+            if (fused) {
+                if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
+                fused->deferred_splits = geo.splits + k_count;
+                fused->deferred_stride = geo.n_pad;
+                return COLATUS_OK;
+            }
+            if (c == 0 && g.profile && geo.chunks == 1) CUDA_TRY(cudaEventRecord(e1, st));
+            if (c == 0)
+                reduce_partials_kernel<false, false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
+                                                                             (float)g.G, eps2, pos_mass, 0, out);
+            else
+                reduce_partials_kernel<false, true><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
+                                                                            (float)g.G, eps2, pos_mass, 0, out);
+            CUDA_TRY(cudaGetLastError());
+            g.launches++;
+        }
+        if (g.profile && geo.chunks > 1) CUDA_TRY(cudaEventRecord(e1, st));
+    } else {
+        const bool single = geo.splits == 1;
+        float4 *fout = single ? out : partials;
+        const float scale = single ? (float)g.G : 1.0f;
+        cudaError_t e = potential ? launch_force<true>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single, fout,
+                                                       t_count, mass_flag, generation, step_ctr, st, fused && fused->pdl)
+                                  : launch_force<false>(geo, pos_mass, packed, t_begin, t_count, eps2, scale, single,
+                                                        fout, t_count, mass_flag, generation, step_ctr, st,
+                                                        fused && fused->pdl);
+        CUDA_TRY(e);
         g.launches++;
+        if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
+
+        if (fused) {
+            fused->deferred_splits = single ? 0 : geo.splits;
+            fused->deferred_stride = t_count;
+            return COLATUS_OK;                      // no external terms in fused steps (checked by the caller)
+        }
+        if (!single) {
+            const unsigned blocks = (unsigned)((t_count + 255) / 256);
+            if (potential)
+                reduce_partials_kernel<true><<<blocks, 256, 0, st>>>(partials, t_count, geo.splits, t_count, (float)g.G,
+                                                                     eps2, pos_mass, t_begin, out);
+            else
+                reduce_partials_kernel<false><<<blocks, 256, 0, st>>>(partials, t_count, geo.splits, t_count,
+                                                                      (float)g.G, eps2, pos_mass, t_begin, out);
+            CUDA_TRY(cudaGetLastError());
+            g.launches++;
+        }
     }
     if (g.def_S != 0.0 || g.bg_rho != 0.0) {   // eq. (10) / background: O(n) epilogue on the finished forces
         const double B = (4.0 * 3.14159265358979323846 / 3.0) * g.G * g.bg_rho;
@@ -387,10 +527,11 @@ int enqueue_step_fused(StepSrc src, cudaStream_t st) {
     const float4 *partials = reinterpret_cast<const float4 *>(g.ws + w.partials);
     if (f.deferred_splits > 0) {
         if (g.trace_k > 0)
-            reduce_kick_drift_kernel<true><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, partials, g.n, f.deferred_splits,
-                                                                   g.n, (float)g.G, f.src, slot, g.ring, g.trace_k);
+            reduce_kick_drift_kernel<true><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, partials, f.deferred_stride,
+                                                                   f.deferred_splits, g.n, (float)g.G, f.src, slot, g.ring,
+                                                                   g.trace_k);
         else
-            reduce_kick_drift_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, partials, g.n,
+            reduce_kick_drift_kernel<false><<<blocks, 256, 0, st>>>(g.pos, g.vel, g.acc, partials, f.deferred_stride,
                                                                     f.deferred_splits, g.n, (float)g.G, f.src, nullptr,
                                                                     nullptr, 0);
     } else if (src.table) {                      // single split: acc is final, plain kick-drift
@@ -464,7 +605,7 @@ int enqueue_step_table(cudaStream_t st) {
 // for the whole run (a captured graph keeps replaying the same value).
 int enqueue_run_head(cudaStream_t st, int generation) {
     const Workspace w = workspace_layout(g.n);
-    const Geometry geo = choose_geometry(g.n, g.n);
+    const Geometry geo = choose_geometry(g.n, g.n, false, true);
     const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
     int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
@@ -496,11 +637,11 @@ int enqueue_step_two_kernels(cudaStream_t st, int generation) {
     cudaError_t e;
     if (g.trace_k > 0)
         e = launch_ex(step_tail_head_kernel<true>, dim3(blocks), dim3(256), 0, st, true, g.pos, g.vel, g.acc, partials,
-                      g.n, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, slot, g.ring, g.trace_k, packed,
+                      f.deferred_stride, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, slot, g.ring, g.trace_k, packed,
                       mass_flag, generation);
     else
         e = launch_ex(step_tail_head_kernel<false>, dim3(blocks), dim3(256), 0, st, true, g.pos, g.vel, g.acc, partials,
-                      g.n, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, (const int32_t *)nullptr,
+                      f.deferred_stride, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, (const int32_t *)nullptr,
                       (float4 *)nullptr, 0, packed, mass_flag, generation);
     CUDA_TRY(e);
     CUDA_TRY(cudaGetLastError());
@@ -558,6 +699,8 @@ int colatus_init(const colatus_config *cfg) {
     g.profile = false;
     g.ev_used = 0;
     g.force_I = g.force_splits = 0;
+    g.symmetric = 1;
+    g.sym_rows = 0;
     g.def_S = g.bg_rho = 0.0;
     invalidate_graph();
     g.initialised = true;
@@ -1083,11 +1226,26 @@ int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]) {
     out[0] = (int64_t)FORCE_THREADS * 2 * geo.IP;
     out[1] = geo.tiles_t;
     out[2] = geo.splits;
-    out[3] = (int64_t)geo.tiles_per_split * geo.TJ;
+    out[3] = geo.sym ? geo.n_pad : (int64_t)geo.tiles_per_split * geo.TJ;
     out[4] = g.ctas_per_sm;
     out[5] = g.sm_count;
     out[6] = 2 * geo.IP;
     out[7] = FORCE_THREADS;
+    return COLATUS_OK;
+}
+
+int colatus_force_plan(int64_t n, int64_t target_count, int with_potential, int64_t out[8]) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!out || n < 1 || target_count < 1 || target_count > n) return fail(COLATUS_INVALID_ARG, "bad arguments");
+    const Geometry geo = choose_geometry(n, target_count, with_potential != 0);
+    out[0] = geo.sym ? 1 : 0;
+    out[1] = geo.sym ? geo.nb : 0;
+    out[2] = geo.splits;
+    out[3] = geo.sym ? geo.H : 0;
+    out[4] = geo.sym ? geo.K : 0;
+    out[5] = geo.sym ? geo.chunks : 1;
+    out[6] = geo.n_pad;
+    out[7] = geo.sym ? geo.splits + (geo.H < geo.K ? geo.H : geo.K) : (geo.splits > 1 ? geo.splits : 0);
     return COLATUS_OK;
 }
 
@@ -1100,6 +1258,12 @@ int colatus_set_option(const char *name, int64_t value) {
     } else if (!strcmp(name, "source_splits")) {
         if (value < 0 || value > MAX_SPLITS) return fail(COLATUS_INVALID_ARG, "must be in [0, %d]", MAX_SPLITS);   // capped per n
         g.force_splits = (int)value;
+    } else if (!strcmp(name, "symmetric")) {
+        if (value < 0 || value > 2) return fail(COLATUS_INVALID_ARG, "must be 0 (never), 1 (automatic) or 2 (always)");
+        g.symmetric = (int)value;
+    } else if (!strcmp(name, "symmetric_rows")) {
+        if (value < 0 || value == 1 || value > 1000000) return fail(COLATUS_INVALID_ARG, "must be 0 or >= 2");
+        g.sym_rows = (int)value;
     } else {
         return fail(COLATUS_INVALID_ARG, "unknown option %s", name);
     }

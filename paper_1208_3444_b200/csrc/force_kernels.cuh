@@ -325,10 +325,30 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
 constexpr int REDUCE_MAX_SPLITS = 64;   // upper bound on source splits (small problems; large ones use <= 16)
 constexpr int REDUCE_CHUNK = 16;        // partials loaded together (held in registers below)
 
-// Sum of the `splits` partials of target t in split order 0, 1, 2, ...: 16 loads at a time (independent, so
+// Sum of the `splits` partials of target t in row order 0, 1, 2, ...: 16 loads at a time (independent, so
 // their latencies overlap), then the adds in fixed order -- the result does not depend on the chunking.
+// Up to REDUCE_MAX_SPLITS rows (the source splits of force_kernel) are added in FP32; more rows (the reaction
+// rows of force_sym_kernel: hundreds) are added in FP64 and rounded once, so the row count does not show in the
+// result's error.  A pure function of (rows, values): every caller gets the same bits.
 __device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partial, int64_t stride, int splits,
                                                int64_t t) {
+    if (splits > REDUCE_MAX_SPLITS) {
+        double sx = 0.0, sy = 0.0, sz = 0.0, sw = 0.0;
+        for (int k0 = 0; k0 < splits; k0 += REDUCE_CHUNK) {
+            float4 q[REDUCE_CHUNK];
+#pragma unroll
+            for (int k = 0; k < REDUCE_CHUNK; ++k)
+                q[k] = k0 + k < splits ? partial[(size_t)(k0 + k) * stride + t] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int k = 0; k < REDUCE_CHUNK; ++k) {
+                sx += (double)q[k].x;
+                sy += (double)q[k].y;
+                sz += (double)q[k].z;
+                sw += (double)q[k].w;
+            }
+        }
+        return make_float4((float)sx, (float)sy, (float)sz, (float)sw);
+    }
     float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int k0 = 0; k0 < splits; k0 += REDUCE_CHUNK) {
         float4 q[REDUCE_CHUNK];
@@ -350,7 +370,8 @@ __device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partia
 }
 
 // ---- fixed-order reduction of the source-split partials, applies G ---------------------------------
-template <bool POT>
+// ACCUM: out[t] += G * sum (later chunks of a chunked symmetric evaluation), else out[t] = G * sum.
+template <bool POT, bool ACCUM = false>
 __global__ void __launch_bounds__(256) reduce_partials_kernel(const float4 *__restrict__ partial, int64_t stride,
                                                              int splits, int64_t t_count, float G, float eps2,
                                                              const float4 *__restrict__ pos_mass, int64_t t_begin,
@@ -363,7 +384,15 @@ __global__ void __launch_bounds__(256) reduce_partials_kernel(const float4 *__re
         const float mk = __ldg(pos_mass + t_begin + t).w;
         pot = -(s.w - mk * rsqrt_approx(eps2)) * G;
     }
-    out[t] = make_float4(s.x * G, s.y * G, s.z * G, pot);
+    float4 r = make_float4(s.x * G, s.y * G, s.z * G, pot);
+    if (ACCUM) {
+        const float4 o = out[t];
+        r.x += o.x;
+        r.y += o.y;
+        r.z += o.z;
+        r.w += o.w;
+    }
+    out[t] = r;
 }
 
 }  // namespace colatus

@@ -1,0 +1,291 @@
+// force_sym_kernels.cuh -- eq. (1) of arXiv 1208.3444 with every pair evaluated ONCE.
+//
+//   F_k = G * sum_{j != k} m_j (x_j - x_k) / (|x_j - x_k|^2 + eps^2)^{3/2}
+//
+// The pair term g_kj = (x_j - x_k) / (r^2 + eps^2)^{3/2} is antisymmetric: body k receives +m_j g_kj and body j
+// receives -m_k g_kj (Newton's third law).  The one-directional kernel of force_kernels.cuh evaluates g twice;
+// this kernel evaluates it once and applies it to both bodies, for whole-range evaluations (targets = sources):
+//
+//   * bodies are cut into NB blocks of BT = 512*IP (the targets one CTA keeps in registers, as in force_kernel);
+//     block a is paired with the H = (NB-1)/2 blocks b = a+1 .. a+H (mod NB) -- a circulant half, so every block
+//     has the same amount of work and every unordered block pair is visited exactly once -- plus, one-directionally
+//     (plain tile body, reaction ignored), with itself and, when NB is even, with the antipodal block a + NB/2;
+//   * inside a symmetric tile the target side accumulates in registers exactly as before; the source side needs
+//     the sum over all targets of the CTA.  Per source a lane first adds up its own 2*IP targets, then the warp
+//     reduces 8 sources at a time with a TRANSPOSED shuffle tree: at unrolled position p lane l works on source
+//     p ^ f(l), f(l) = (l >> 2) & 7, so at every level of the tree the value to keep and the value to send sit in
+//     fixed registers (no selects): v[p] += shfl_xor(v[p + h], 4h), h = 4, 2, 1, then two full levels (xor 2, 1).
+//     9 shuffles + 9 adds per component per 8 sources; the order is fixed, so results are reproducible bit for bit;
+//   * per-warp reaction sums live in shared memory (private to the warp), are added over the 8 warps in fixed
+//     order at the end of the tile and written to a row of their own: row S + k - 1 for block distance k.  The
+//     fixed-order sum over the S target-side rows and the H reaction rows is the existing partial-sum reduction.
+//
+// FMA-pipe work per pair: 16 packed ops per (target pair, source) = 4 pair-interactions (14 for equal masses)
+// against 24 (22) for two one-directional evaluations.
+#pragma once
+#include "force_kernels.cuh"
+
+namespace colatus {
+
+template <int IP, int TJ, int NST>
+constexpr size_t force_sym_smem_bytes() {
+    return (size_t)NST * TJ * 16 + 2 * NST * sizeof(uint64_t) + (size_t)IP * 3 * FORCE_THREADS * 8 +
+           (size_t)3 * (FORCE_THREADS / 32) * TJ * 4;
+}
+
+// One source tile against the thread's target pairs, both directions.  racc = this warp's reaction sums
+// [3][TJ] (x, y, z rows).  mi = the masses of the thread's own target pairs (general loop only).
+template <int IP, int TJ, bool EQM>
+__device__ __forceinline__ void sym_tile_body(const unsigned char *tile, const u64 (&nx)[IP], const u64 (&ny)[IP],
+                                              const u64 (&nz)[IP], const u64 (&mi)[IP], u64 eps2_2, u64 (&ax)[IP],
+                                              u64 (&ay)[IP], u64 (&az)[IP], float *racc, int lane) {
+    const int f = (lane >> 2) & 7;
+    for (int jb = 0; jb < TJ; jb += 8) {
+        float vx[8], vy[8], vz[8];
+#pragma unroll
+        for (int p = 0; p < 8; ++p) {
+            // (p ^ f) * 16 == (p * 16) ^ (f * 16); tile rows of 8 sources are 128-byte aligned
+            const float4 S = *reinterpret_cast<const float4 *>(
+                tile + (((jb + p) << 4) ^ (f << 4)));
+            const u64 X = pack2(S.x, S.x), Y = pack2(S.y, S.y), Z = pack2(S.z, S.z), M = pack2(S.w, S.w);
+            u64 rx = 0ull, ry = 0ull, rz = 0ull;
+#pragma unroll
+            for (int i = 0; i < IP; ++i) {
+                const u64 dx = add2(nx[i], X);
+                const u64 dy = add2(ny[i], Y);
+                const u64 dz = add2(nz[i], Z);
+                u64 r2 = fma2(dz, dz, eps2_2);
+                r2 = fma2(dy, dy, r2);
+                r2 = fma2(dx, dx, r2);
+                float r2a, r2b;
+                unpack2(r2, r2a, r2b);
+                const u64 rinv = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));
+                const u64 rinv2 = mul2(rinv, rinv);
+                const u64 r3 = mul2(rinv, rinv2);
+                const u64 wi = EQM ? r3 : mul2(r3, M);
+                const u64 wj = EQM ? r3 : mul2(r3, mi[i]);
+                ax[i] = fma2(wi, dx, ax[i]);
+                rx = fma2(wj, dx, rx);
+                ry = fma2(wj, dy, ry);
+                ay[i] = fma2(wi, dy, ay[i]);
+                az[i] = fma2(wi, dz, az[i]);
+                rz = fma2(wj, dz, rz);
+            }
+            float lo, hi;
+            unpack2(rx, lo, hi);
+            vx[p] = lo + hi;
+            unpack2(ry, lo, hi);
+            vy[p] = lo + hi;
+            unpack2(rz, lo, hi);
+            vz[p] = lo + hi;
+        }
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            vx[p] += __shfl_xor_sync(0xffffffffu, vx[p + 4], 16);
+            vy[p] += __shfl_xor_sync(0xffffffffu, vy[p + 4], 16);
+            vz[p] += __shfl_xor_sync(0xffffffffu, vz[p + 4], 16);
+        }
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            vx[p] += __shfl_xor_sync(0xffffffffu, vx[p + 2], 8);
+            vy[p] += __shfl_xor_sync(0xffffffffu, vy[p + 2], 8);
+            vz[p] += __shfl_xor_sync(0xffffffffu, vz[p + 2], 8);
+        }
+        vx[0] += __shfl_xor_sync(0xffffffffu, vx[1], 4);
+        vy[0] += __shfl_xor_sync(0xffffffffu, vy[1], 4);
+        vz[0] += __shfl_xor_sync(0xffffffffu, vz[1], 4);
+        vx[0] += __shfl_xor_sync(0xffffffffu, vx[0], 2);
+        vy[0] += __shfl_xor_sync(0xffffffffu, vy[0], 2);
+        vz[0] += __shfl_xor_sync(0xffffffffu, vz[0], 2);
+        vx[0] += __shfl_xor_sync(0xffffffffu, vx[0], 1);
+        vy[0] += __shfl_xor_sync(0xffffffffu, vy[0], 1);
+        vz[0] += __shfl_xor_sync(0xffffffffu, vz[0], 1);
+        if ((lane & 3) == 0) {                           // lane l now holds the warp's sum for source jb + f(l)
+            racc[jb + f] += vx[0];
+            racc[TJ + jb + f] += vy[0];
+            racc[2 * TJ + jb + f] += vz[0];
+        }
+    }
+}
+
+// Position p of block a's tile list in one launch -> (source tile index, block distance k; k = 0: plain tile).
+// A launch covers the block distances k_begin .. k_begin + k_count - 1 and, if `with_plain`, the one-directional
+// blocks (the block itself first, the antipodal block last when NB is even).
+struct SymTile {
+    int tile;   // index of the TJ-source tile in the staged array
+    int k;      // 0 = one-directional (diagonal or antipodal block), else symmetric with block distance k
+    int sub;    // tile within the block
+};
+template <int TPB>
+__device__ __forceinline__ SymTile sym_tile_at(int p, int a, int nb, int k_begin, int k_count, int with_plain) {
+    SymTile t;
+    const int lead = with_plain ? TPB : 0;
+    int b;
+    if (p < lead) {
+        t.k = 0;
+        t.sub = p;
+        b = a;
+    } else if (p < lead + TPB * k_count) {
+        const int q = p - lead;
+        const int dk = q / TPB;
+        t.k = k_begin + dk;
+        t.sub = q - dk * TPB;
+        b = a + t.k;
+    } else {
+        t.k = 0;
+        t.sub = p - lead - TPB * k_count;
+        b = a + nb / 2;
+    }
+    if (b >= nb) b -= nb;
+    t.tile = b * TPB + t.sub;
+    return t;
+}
+
+// grid = (NB blocks, S splits).  staged = the source array padded to NB * BT bodies (far-away zero-mass padding);
+// targets are read from it too.  Split s works on positions [s * P / S, (s + 1) * P / S) of the block's list of
+// P = TPB * (k_count + (with_plain ? 1 + (NB even) : 0)) tiles.  Output rows of `stride` float4: row s =
+// target-side sums of split s (all NB * BT targets); row S + (k - k_begin) = reaction sums (already negated) of
+// block distance k.  Every row is written in full by every launch.
+template <int IP, int TJ, int NST, int MINB>
+__global__ void __launch_bounds__(FORCE_THREADS, MINB)
+force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_begin, int k_count, int with_plain,
+                 float eps2, float4 *__restrict__ partial, int64_t stride, const int *__restrict__ mass_flag,
+                 int generation, int *__restrict__ step_ctr) {
+    constexpr int TILE_BYTES = TJ * 16;
+    constexpr int BT = FORCE_THREADS * 2 * IP;
+    constexpr int TPB = BT / TJ;
+    constexpr int NW = FORCE_THREADS / 32;
+    static_assert(BT % TJ == 0, "a block is a whole number of tiles");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem_raw + NST * TILE_BYTES);
+    uint64_t *empty_bar = full_bar + NST;
+    u64 *acc2 = reinterpret_cast<u64 *>(smem_raw + NST * TILE_BYTES + 2 * NST * 8);   // [IP*3][THREADS]
+    float *racc_all = reinterpret_cast<float *>(acc2 + (size_t)IP * 3 * FORCE_THREADS);   // [NW][3][TJ]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int a = blockIdx.x, s = blockIdx.y;
+    const int P = TPB * (k_count + (with_plain ? ((nb & 1) ? 1 : 2) : 0));
+    const int p0 = (int)(((int64_t)s * P) / splits), p1 = (int)(((int64_t)(s + 1) * P) / splits);
+    const unsigned char *src = reinterpret_cast<const unsigned char *>(staged);
+
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NST; ++q) {
+            mbar_init(&full_bar[q], 1);
+            mbar_init(&empty_bar[q], NW);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    griddep_wait();
+    griddep_launch_dependents();
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NST; ++q)
+            if (p0 + q < p1) {
+                const SymTile t = sym_tile_at<TPB>(p0 + q, a, nb, k_begin, k_count, with_plain);
+                mbar_arrive_expect_tx(&full_bar[q], TILE_BYTES);
+                bulk_copy_g2s(smem_raw + q * TILE_BYTES, src + (size_t)t.tile * TILE_BYTES, TILE_BYTES, &full_bar[q]);
+            }
+    }
+
+    u64 nx[IP], ny[IP], nz[IP], mi[IP];
+    const int64_t tbase = (int64_t)a * BT + 2 * tid;
+#pragma unroll
+    for (int i = 0; i < IP; ++i) {
+        const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
+        const float4 b0 = __ldg(staged + t), b1 = __ldg(staged + t + 1);
+        nx[i] = pack2(-b0.x, -b1.x);
+        ny[i] = pack2(-b0.y, -b1.y);
+        nz[i] = pack2(-b0.z, -b1.z);
+        mi[i] = pack2(b0.w, b1.w);
+    }
+    const u64 eps2_2 = pack2(eps2, eps2);
+#pragma unroll
+    for (int c = 0; c < IP * 3; ++c) acc2[c * FORCE_THREADS + tid] = 0ull;
+    float *racc = racc_all + (size_t)warp * 3 * TJ;
+    for (int j = lane; j < 3 * TJ; j += 32) racc[j] = 0.f;
+    if (step_ctr && tid == FORCE_THREADS - 1 && a == 0 && s == 0) step_ctr[1] = step_ctr[0];
+    const bool eqm = __ldg(mass_flag) != generation;
+    const float m_common = eqm ? __ldg(staged).w : 1.0f;        // applied once to the finished sums
+    __syncwarp();
+
+    for (int p = p0; p < p1; ++p) {
+        const int it = p - p0;
+        const int stage = it % NST;
+        const uint32_t parity = (it / NST) & 1;
+        const SymTile T = sym_tile_at<TPB>(p, a, nb, k_begin, k_count, with_plain);
+        mbar_wait(&full_bar[stage], parity);
+        const unsigned char *tile = smem_raw + (size_t)stage * TILE_BYTES;
+        u64 ax[IP], ay[IP], az[IP], ap[IP];
+#pragma unroll
+        for (int i = 0; i < IP; ++i) ax[i] = ay[i] = az[i] = ap[i] = 0ull;
+        if (T.k == 0) {
+            const float4 *tp = reinterpret_cast<const float4 *>(tile);
+            if (eqm)
+                force_tile_body<IP, TJ, false, true>(tp, nx, ny, nz, eps2_2, ax, ay, az, ap);
+            else
+                force_tile_body<IP, TJ, false, false>(tp, nx, ny, nz, eps2_2, ax, ay, az, ap);
+        } else {
+            if (eqm)
+                sym_tile_body<IP, TJ, true>(tile, nx, ny, nz, mi, eps2_2, ax, ay, az, racc, lane);
+            else
+                sym_tile_body<IP, TJ, false>(tile, nx, ny, nz, mi, eps2_2, ax, ay, az, racc, lane);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[stage]);
+        if (tid == 0 && p + NST < p1) {
+            const SymTile N = sym_tile_at<TPB>(p + NST, a, nb, k_begin, k_count, with_plain);
+            mbar_wait(&empty_bar[stage], parity);
+            mbar_arrive_expect_tx(&full_bar[stage], TILE_BYTES);
+            bulk_copy_g2s(smem_raw + stage * TILE_BYTES, src + (size_t)N.tile * TILE_BYTES, TILE_BYTES,
+                          &full_bar[stage]);
+        }
+#pragma unroll
+        for (int i = 0; i < IP; ++i) {
+            u64 *a2 = acc2 + (size_t)(i * 3) * FORCE_THREADS + tid;
+            a2[0] = add2(a2[0], ax[i]);
+            a2[FORCE_THREADS] = add2(a2[FORCE_THREADS], ay[i]);
+            a2[2 * FORCE_THREADS] = add2(a2[2 * FORCE_THREADS], az[i]);
+        }
+        if (T.k != 0) {
+            // reaction of this tile: add the 8 warps' sums in warp order, negate, write the row of distance k
+            __syncthreads();
+            int bb = a + T.k;
+            if (bb >= nb) bb -= nb;
+            float4 *row = partial + (size_t)(splits + T.k - k_begin) * stride + (size_t)bb * BT + (size_t)T.sub * TJ;
+            for (int j = tid; j < TJ; j += FORCE_THREADS) {
+                float sx = racc_all[j], sy = racc_all[TJ + j], sz = racc_all[2 * TJ + j];
+#pragma unroll
+                for (int w = 1; w < NW; ++w) {
+                    sx += racc_all[(size_t)w * 3 * TJ + j];
+                    sy += racc_all[(size_t)w * 3 * TJ + TJ + j];
+                    sz += racc_all[(size_t)w * 3 * TJ + 2 * TJ + j];
+                }
+                row[j] = make_float4(-sx * m_common, -sy * m_common, -sz * m_common, 0.f);
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    racc_all[(size_t)w * 3 * TJ + j] = 0.f;
+                    racc_all[(size_t)w * 3 * TJ + TJ + j] = 0.f;
+                    racc_all[(size_t)w * 3 * TJ + 2 * TJ + j] = 0.f;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    float4 *o = partial + (size_t)s * stride;
+#pragma unroll
+    for (int i = 0; i < IP; ++i) {
+        const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
+        const u64 *a2 = acc2 + (size_t)(i * 3) * FORCE_THREADS + tid;
+        float fx[2], fy[2], fz[2];
+        unpack2(a2[0], fx[0], fx[1]);
+        unpack2(a2[FORCE_THREADS], fy[0], fy[1]);
+        unpack2(a2[2 * FORCE_THREADS], fz[0], fz[1]);
+        o[t] = make_float4(fx[0] * m_common, fy[0] * m_common, fz[0] * m_common, 0.f);
+        o[t + 1] = make_float4(fx[1] * m_common, fy[1] * m_common, fz[1] * m_common, 0.f);
+    }
+}
+
+}  // namespace colatus

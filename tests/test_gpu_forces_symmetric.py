@@ -1,0 +1,197 @@
+"""The symmetric force kernel (every pair once, Newton's third law; force_sym_kernels.cuh, colatus_force_plan)
+against the FP64 oracle, through the C ABI.  It is picked automatically for whole-range evaluations of at least
+49152 bodies (configs 3-5: covered at full size in test_gpu_forces.py); here it is forced on at small and ragged
+sizes so that every structural case is hit: 1 block (diagonal only), 2 blocks (antipodal only), odd and even
+block counts, ragged last blocks, every split count, equal and general masses, chunked evaluations.
+Tolerances: north_star's (G17), as in test_gpu_forces.py."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+from paper_1208_3444_b200 import binding as B  # noqa: E402
+from paper_1208_3444_b200 import inputs  # noqa: E402
+from conftest import record_parity  # noqa: E402
+from test_gpu_forces import MAX_TOL, MEDIAN_TOL, force_errors  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def session():
+    from paper_1208_3444_b200.harness import Session
+    s = Session(1.0, 1 << 18)
+    yield s
+    s.close()
+
+
+@pytest.fixture()
+def symmetric_always():
+    B.colatus_set_option("symmetric", 2)
+    yield
+    B.colatus_set_option("symmetric", 1)
+    B.colatus_set_option("symmetric_rows", 0)
+    B.colatus_set_option("source_splits", 0)
+
+
+def _problem(n, equal_mass, seed=0):
+    rng = np.random.Generator(np.random.PCG64(9100 + seed))
+    pm = np.empty((n, 4), dtype=np.float32)
+    half = n // 2
+    pm[:half, :3] = rng.random((half, 3))
+    pm[half:, :3] = 0.5 + 0.03 * rng.standard_normal((n - half, 3))          # a clump: close pairs
+    pm[:, 3] = 1.0 / n if equal_mass else np.exp(0.5 * rng.standard_normal(n)) / n
+    return pm[rng.permutation(n)]
+
+
+@pytest.mark.parametrize("equal_mass", [False, True])
+@pytest.mark.parametrize("n", [1, 2, 3, 1535, 1536, 1537, 3072, 3073, 4609, 6145, 7000, 10753, 12289])
+def test_symmetric_kernel_ragged_sizes(session, symmetric_always, n, equal_mass):
+    """blocks = 1 (diagonal only), 2 (antipodal only), 3, 4, 5, 7, 8, 9: odd and even counts, full and ragged
+    last blocks; all targets against the oracle."""
+    pm = _problem(n, equal_mass, seed=n)
+    eps2 = np.float32(1e-4)
+    plan = B.colatus_force_plan(n)
+    assert plan["symmetric"] == 1 and plan["blocks"] == (n + 1535) // 1536
+    assert plan["distances"] == (plan["blocks"] - 1) // 2
+    out = session.forces(pm, eps2).cpu().numpy()
+    assert np.all(out[:, 3] == 0.0)
+    if n == 1:
+        assert np.all(out == 0.0)
+        return
+    ref = oracle.forces(pm, eps2, 1.0)
+    med, mx = force_errors(out[:, :3], ref)
+    record_parity(f"symmetric kernel n={n} equal_mass={equal_mass}", n=n, targets=n, median_rel=med, max_over_rms=mx)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (n, equal_mass, med, mx)
+
+
+@pytest.mark.parametrize("splits", [1, 2, 3, 5, 7, 16])
+def test_symmetric_kernel_split_counts(session, symmetric_always, splits):
+    """Any split of a block's tile list (a split may begin or end inside a block, and may be empty)."""
+    n = 13000                                                        # 9 blocks, H = 4: 15 tiles per block
+    pm = _problem(n, False, seed=splits)
+    eps2 = np.float32(2.5e-5)
+    B.colatus_set_option("source_splits", splits)
+    plan = B.colatus_force_plan(n)
+    assert plan["symmetric"] == 1 and plan["splits"] == splits
+    out = session.forces(pm, eps2).cpu().numpy()
+    ref = oracle.forces(pm, eps2, 1.0)
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (splits, med, mx)
+
+
+def test_symmetric_kernel_chunked_evaluation(session, symmetric_always):
+    """A cap on the partial rows per launch splits the block distances over several launches whose sums are
+    accumulated: same forces (to rounding) as the single launch, and the oracle's."""
+    n = 30000                                                        # 20 blocks, H = 9, antipodal block
+    pm = _problem(n, False, seed=77)
+    eps2 = np.float32(1e-5)
+    B.colatus_set_option("source_splits", 3)
+    one = session.forces(pm, eps2).cpu().numpy()
+    assert B.colatus_force_plan(n)["launches"] == 1
+    ref = oracle.forces(pm, eps2, 1.0)
+    for rows, launches in ((3 + 4, 3), (3 + 1, 9), (3 + 5, 2)):
+        B.colatus_set_option("symmetric_rows", rows)
+        plan = B.colatus_force_plan(n)
+        assert plan["launches"] == launches and plan["distances_per_launch"] == rows - 3, plan
+        out = session.forces(pm, eps2).cpu().numpy()
+        med, mx = force_errors(out[:, :3], ref)
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL, (rows, med, mx)
+        assert np.abs(out - one).max() <= 2e-6 * np.abs(one).max()
+
+
+def test_symmetric_kernel_matches_one_directional_kernel(session, symmetric_always):
+    """Same problem through both kernels: equal to FP32 summation rounding, both within the bars; the symmetric
+    result obeys Newton's third law to rounding (sum m F = 0), and is bitwise reproducible."""
+    cfg, pm, _ = inputs.make_config(3, n_override=40000)
+    sym = session.forces(pm, cfg.eps2).cpu().numpy()
+    again = session.forces(pm, cfg.eps2).cpu().numpy()
+    assert np.array_equal(sym, again)
+    B.colatus_set_option("symmetric", 0)
+    assert B.colatus_force_plan(cfg.n)["symmetric"] == 0
+    plain = session.forces(pm, cfg.eps2).cpu().numpy()
+    ref = oracle.forces(pm, cfg.eps2, 1.0)
+    for name, out in (("symmetric", sym), ("one-directional", plain)):
+        med, mx = force_errors(out[:, :3], ref)
+        record_parity(f"config-3-shaped n=40000 {name} kernel", n=cfg.n, targets=cfg.n, median_rel=med, max_over_rms=mx)
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL, (name, med, mx)
+    m = pm[:, 3].astype(np.float64)
+    F = sym[:, :3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * F).sum(0)) / (m * np.linalg.norm(F, axis=1)).sum() < 2e-6
+
+
+def test_symmetric_kernel_masses(session, symmetric_always):
+    """Equal-mass detection inside the symmetric kernel: one different mass (also 0) is honoured; all-zero masses
+    give exact zeros; a NaN mass gives NaN forces, not an error."""
+    n = 5000
+    pm0 = _problem(n, True, seed=5)
+    eps2 = np.float32(1e-4)
+    for where, factor in ((0, 3.0), (2500, 0.0), (4999, 50.0)):
+        pm = pm0.copy()
+        pm[where, 3] *= factor
+        out = session.forces(pm, eps2).cpu().numpy()
+        ref = oracle.forces(pm, eps2, 1.0)
+        med, mx = force_errors(out[:, :3], ref)
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL, (where, factor, med, mx)
+    z = pm0.copy()
+    z[:, 3] = 0.0
+    assert np.all(session.forces(z, eps2).cpu().numpy() == 0.0)
+    q = pm0.copy()
+    q[7, 3] = np.nan
+    out = session.forces(q, eps2).cpu().numpy()
+    assert np.isnan(out[:, :3]).all(axis=1).sum() >= n - 1
+
+
+def test_symmetric_kernel_at_the_smallest_accepted_eps2(session, symmetric_always):
+    """Coincident bodies and the eps2 floor (reading G4): the pair term of coincident bodies is exactly 0 in both
+    directions."""
+    n = 4000
+    pm = _problem(n, False, seed=11)
+    pm[100, :3] = pm[3000, :3]                                       # two coincident bodies in different blocks
+    pm[200, :3] = pm[201, :3]                                        # ... and in the same block
+    eps2 = np.float32(1e-24)
+    out = session.forces(pm, eps2).cpu().numpy()
+    assert np.isfinite(out).all()
+    ref = oracle.forces(pm, eps2, 1.0)
+    med, mx = force_errors(out[:, :3], ref)
+    assert med <= MEDIAN_TOL and mx <= MAX_TOL, (med, mx)
+
+
+def test_symmetric_steps_match_the_oracle_and_the_run_loop(session, symmetric_always):
+    """10 steps of config 1 with the symmetric kernel inside colatus_step (fused kick) and inside colatus_run
+    (two-kernel loop, graphs): the 10-step bar against the oracle (G16), and run == step loop bit for bit."""
+    cfg, pm, vel = inputs.make_config(1)
+    assert cfg.G == 1.0
+    s = session
+    if True:
+        assert B.colatus_force_plan(cfg.n)["symmetric"] == 1
+        steps = 10
+        mids, _ = oracle.midstep_schedule(cfg.cosmo, cfg.a_start, cfg.tau, steps)
+        s.upload(pm, vel, cfg.eps2)
+        s.run(cfg.cosmo, cfg.a_start, cfg.tau, steps)
+        pos_a, vel_a = s.download()
+        st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+        for a, H in mids:
+            st.step(cfg.tau, a, H)
+        dx = float(np.linalg.norm(pos_a[:, :3].astype(np.float64) - st.x, axis=1).max())
+        assert dx <= 1e-5, dx
+        for use_graph in (False, True):
+            s.upload(pm, vel, cfg.eps2)
+            s.run_native(cfg.cosmo, cfg.a_start, cfg.tau, steps, use_graph=use_graph)
+            pos_b, vel_b = s.download()
+            assert np.array_equal(pos_a, pos_b) and np.array_equal(vel_a, vel_b), use_graph
+
+
+def test_plan_of_the_baseline_configurations(session):
+    """What colatus_force_plan reports for BASELINE.json's sizes on this device."""
+    if True:
+        small = B.colatus_force_plan(32768)
+        assert small["symmetric"] == 0
+        for n in (131072, 1 << 20):
+            p = B.colatus_force_plan(n)
+            assert p["symmetric"] == 1 and p["launches"] == 1 and p["blocks"] == (n + 1535) // 1536
+            assert p["partial_rows"] == p["splits"] + p["distances"]
+        big = B.colatus_force_plan(1 << 22)
+        assert big["symmetric"] == 1 and big["launches"] > 1
+        assert big["partial_rows"] * big["padded_bodies"] * 16 <= 8 << 30
+        assert B.colatus_force_plan(1 << 20, 1 << 19)["symmetric"] == 0          # target sub-range
+        assert B.colatus_force_plan(1 << 20, None, True)["symmetric"] == 0       # potential
