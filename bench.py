@@ -40,12 +40,18 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
 FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
 # dram__bytes_read.sum + dram__bytes_write.sum of one force-kernel launch from the `ncu --set full` capture
 # summarised in profiles/: valid only for the (n, source splits) it was captured at -- reported as null otherwise.
-FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8,
+FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8, "symmetric": 0,
                              "profile": "profiles/r02_force_kernel_ncu_full.txt"}
+SYM_KERNEL_DRAM_TRAFFIC = None             # filled from the ncu --set full capture of force_sym_kernel (profiles/)
 # executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
 # (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention
 EXECUTED_FLOP_GENERAL, EXECUTED_FLOP_EQUAL_MASS = 19.0, 18.0
 FMA_PIPE_LANE_OPS_GENERAL, FMA_PIPE_LANE_OPS_EQUAL_MASS = 12.0, 11.0
+# symmetric kernel (each unordered pair once, applied to both bodies): per PAIR 3 add + 3 fma + rsqrt
+# + 4 mul (2 for equal masses) + 6 fma = 26 (24) flop and 16 (14) FMA-pipe lane-ops, plus ~1.07 adds per pair for
+# the reaction reduction (6.4 scalar adds per source and lane, 6 targets per lane); a pair is TWO interactions
+SYM_EXECUTED_FLOP_GENERAL, SYM_EXECUTED_FLOP_EQUAL_MASS = (26.0 + 1.07) / 2, (24.0 + 1.07) / 2
+SYM_LANE_OPS_GENERAL, SYM_LANE_OPS_EQUAL_MASS = (16.0 + 1.07) / 2, (14.0 + 1.07) / 2
 METRIC = "Ginteractions/s softened direct-sum gravity at N=2^20; % of FP32 FMA peak"
 UNIT = "Ginteractions/s"
 BENCH_TAU = 1.0e-6                         # step size of the bench steps (EdS background from a = 0.02)
@@ -300,27 +306,49 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
     # ---- roofline of the dominant kernel (force kernel), from events inside the timed region
     pairs_per_launch = float(count) * n
     geo = B.colatus_force_geometry(n, count)
+    plan = B.colatus_force_plan(n, count)
+    geo["plan"] = plan
+    sym = bool(plan["symmetric"])
     equal_mass = bool(np.all(pm[:, 3] == pm[0, 3]))
     k_ms = kernel_ms / max(kernel_launches, 1)
     per_s = pairs_per_launch / (k_ms * 1e-3)
     achieved = FLOP_PER_INTERACTION * per_s / 1e12
-    cap = FORCE_KERNEL_DRAM_TRAFFIC
-    traffic = cap["bytes"] if (n == cap["n"] and world == 1 and geo["source_splits"] == cap["splits"]) else None
-    lane_ops = FMA_PIPE_LANE_OPS_EQUAL_MASS if equal_mass else FMA_PIPE_LANE_OPS_GENERAL
+    if sym:
+        cap = SYM_KERNEL_DRAM_TRAFFIC
+        traffic = cap["bytes"] if (cap and n == cap["n"] and world == 1 and plan["splits"] == cap["splits"]) else None
+        lane_ops = SYM_LANE_OPS_EQUAL_MASS if equal_mass else SYM_LANE_OPS_GENERAL
+        executed = SYM_EXECUTED_FLOP_EQUAL_MASS if equal_mass else SYM_EXECUTED_FLOP_GENERAL
+        # staged bodies read as targets and as sources, every partial row written once
+        algorithmic_bytes = 16 * plan["padded_bodies"] * (2 + plan["splits"] + plan["distances"])
+        kernel = "force_sym_kernel<3,512,4,2> (every pair once, applied to both bodies)%s%s" % (
+            " equal-mass loop" if equal_mass else "",
+            "; %d launches + partial-row reductions per evaluation" % plan["launches"] if plan["launches"] > 1 else "")
+    else:
+        cap = FORCE_KERNEL_DRAM_TRAFFIC
+        traffic = cap["bytes"] if (n == cap["n"] and world == 1 and geo["source_splits"] == cap["splits"]) else None
+        lane_ops = FMA_PIPE_LANE_OPS_EQUAL_MASS if equal_mass else FMA_PIPE_LANE_OPS_GENERAL
+        executed = EXECUTED_FLOP_EQUAL_MASS if equal_mass else EXECUTED_FLOP_GENERAL
+        algorithmic_bytes = 16 * n * (2 + (geo["source_splits"] if geo["source_splits"] > 1 else 0))
+        kernel = "force_kernel<%d,%d,4,false,2>%s" % (geo["targets_per_thread"] // 2,
+                                                      {6: 512, 4: 512, 2: 128}[geo["targets_per_thread"]],
+                                                      " equal-mass loop" if equal_mass else "")
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
                 "traffic_from": cap["profile"] if traffic else None,
-                "algorithmic_bytes": 16 * n * (2 + (geo["source_splits"] if geo["source_splits"] > 1 else 0)),
-                "kernel": "force_kernel<%d,%d,4,false,2>%s" % (geo["targets_per_thread"] // 2,
-                                                                 {6: 512, 4: 512, 2: 128}[geo["targets_per_thread"]],
-                                                                 " equal-mass loop" if equal_mass else ""),
+                "algorithmic_bytes": algorithmic_bytes,
+                "kernel": kernel,
                 "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / ms_step,
                 "peak_basis": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (DESIGN.md); "
                               "no FP32 figure in MEASURED_PEAKS.json",
                 "flop_per_interaction": FLOP_PER_INTERACTION,
-                "frac_executed_flops": (EXECUTED_FLOP_EQUAL_MASS if equal_mass else EXECUTED_FLOP_GENERAL) * per_s
-                                       / 1e12 / FP32_PEAK_TFLOPS,
+                "frac_note": ("achieved = ALGORITHMIC flops: 20 flop x N^2 pair interactions delivered / kernel time "
+                              "(BASELINE convention)." + (" The symmetric kernel evaluates each unordered pair once "
+                              "and applies it to both bodies, so it EXECUTES ~13.5 flop per delivered interaction: "
+                              "frac can exceed 20/24 = 0.833, the ceiling of a one-directional kernel; "
+                              "frac_executed_flops and fma_pipe_busy_frac count what the SMs really did."
+                              if sym else "")),
+                "frac_executed_flops": executed * per_s / 1e12 / FP32_PEAK_TFLOPS,
                 "fma_pipe_busy_frac": lane_ops * per_s / (SM_COUNT * FP32_LANES * SM_MAX_MHZ * 1e6),
                 "frac_at_sampled_clock": (achieved / (FP32_PEAK_TFLOPS * clocks["sm_mhz"] / SM_MAX_MHZ)
                                           if clocks.get("sm_mhz") else None)}

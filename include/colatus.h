@@ -287,7 +287,7 @@ int64_t  colatus_launch_count(void);
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 
 /* Which force kernel an evaluation of target_count targets out of n bodies takes (eq. 1).
- * Whole-range evaluations (target_count == n) without the potential and with at least 49152 bodies use the
+ * Whole-range evaluations (target_count == n) without the potential and with at least 24576 bodies use the
  * SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
  * per unordered pair and applied to both bodies (Newton's third law) -- 16 packed FP32 operations per
  * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 1536; block a meets the `distances`

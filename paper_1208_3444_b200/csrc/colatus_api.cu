@@ -34,8 +34,9 @@ constexpr int GRAPH_STEPS = 8;        // steps per replay of the multi-step grap
 constexpr int SYM_IP = 3, SYM_TJ = 512;
 constexpr int64_t SYM_BT = (int64_t)FORCE_THREADS * 2 * SYM_IP;   // bodies per block = targets of one CTA
 constexpr int SYM_TPB = (int)(SYM_BT / SYM_TJ);                   // tiles per block
-constexpr int64_t SYM_MIN_N = 49152;
+constexpr int64_t SYM_MIN_N = 24576;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
 constexpr int SYM_MAX_SPLITS = 16;
+constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)
 constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch can always hold
 constexpr size_t SYM_ROWS_BUDGET = (size_t)8 << 30;               // bytes of partial rows before an evaluation is chunked
 
@@ -272,18 +273,23 @@ Geometry choose_sym_geometry(int64_t n) {
     return geo;
 }
 
-Geometry choose_geometry(int64_t n, int64_t t_count, bool potential = false, bool single_launch = false) {
+Geometry choose_geometry(int64_t n, int64_t t_count, bool potential = false) {
     if (sym_eligible(n, t_count, potential)) {
         const Geometry geo = choose_sym_geometry(n);
-        if (geo.sym && (!single_launch || geo.chunks == 1)) return geo;
+        if (geo.sym) return geo;
     }
     return choose_plain_geometry(n, t_count);
 }
 
-cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
-                             float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
-                             cudaStream_t st, bool pdl) {
-    auto kern = force_sym_kernel<SYM_IP, SYM_TJ, NSTAGES, 2>;
+// One evaluation chunk = one launch of the kernel that holds both tile bodies (general, equal-mass; picked on the
+// device), or -- from SYM_PAIR_N bodies on -- two launches, a general-only and an equal-mass-only kernel, of which the
+// one the equal-mass flag does not ask for returns at once (15 us at 2^20): compiled alone the general body runs
+// 2.4 % faster (94.0 % against 91.8 % of peak at 2^20; the equal-mass body is the same either way).
+template <int BODY>
+cudaError_t launch_force_sym_body(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
+                                  float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
+                                  cudaStream_t st, bool pdl) {
+    auto kern = force_sym_kernel<SYM_IP, SYM_TJ, NSTAGES, 2, BODY>;
     const size_t smem = force_sym_smem_bytes<SYM_IP, SYM_TJ, NSTAGES>();
     static int attr_epoch = 0;
     if (attr_epoch != g.init_epoch) {
@@ -294,6 +300,22 @@ cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_be
     dim3 grid((unsigned)geo.nb, (unsigned)geo.splits);
     return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, packed, geo.nb, geo.splits, k_begin, k_count,
                      with_plain, eps2, partials, geo.n_pad, mass_flag, generation, step_ctr);
+}
+
+inline bool sym_pair(const Geometry &geo) { return geo.n_pad >= SYM_PAIR_N; }
+
+cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
+                             float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
+                             cudaStream_t st, bool pdl) {
+    if (!sym_pair(geo))
+        return launch_force_sym_body<0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
+                                        generation, step_ctr, st, pdl);
+    cudaError_t e = launch_force_sym_body<1>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
+                                             generation, step_ctr, st, pdl);
+    if (e != cudaSuccess) return e;
+    g.launches++;
+    return launch_force_sym_body<2>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag, generation,
+                                    step_ctr, st, pdl);
 }
 
 template <int IP, int TJ, bool POT>
@@ -355,7 +377,7 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     if (w.total > g.ws_bytes)
         return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
                     (long long)n, w.total);
-    const Geometry geo = choose_geometry(n, t_count, potential, fused != nullptr);
+    const Geometry geo = choose_geometry(n, t_count, potential);
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
     float4 *partials = reinterpret_cast<float4 *>(g.ws + w.partials);
 
@@ -399,16 +421,17 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     int *step_ctr = fused ? fused->step_ctr : nullptr;
     if (geo.sym) {
         // every pair once (force_sym_kernels.cuh): one launch per chunk of block distances; its rows (target-side
-        // sums of the splits, then one reaction row per distance) are added in row order by the reduction -- here,
-        // or inside the caller's fused kick kernel (single-chunk geometries only)
+        // sums of the splits, then one reaction row per distance) are added in row order by the reduction -- inside
+        // the caller's fused kick kernel when one launch covers all distances, else here, chunk after chunk into
+        // `out` (a fused caller is then told that `out` is final: deferred_splits = 0)
         const unsigned blocks = (unsigned)((n + 255) / 256);
         for (int c = 0; c < geo.chunks; ++c) {
             const int k_begin = 1 + c * geo.K;
             const int k_count = geo.H - c * geo.K < geo.K ? geo.H - c * geo.K : geo.K;
             CUDA_TRY(launch_force_sym(geo, packed, k_begin, k_count, c == 0, eps2, partials, mass_flag, generation,
-                                      c == 0 ? step_ctr : nullptr, st, fused && fused->pdl));
+                                      c == 0 ? step_ctr : nullptr, st, fused && fused->pdl && c == 0));
             g.launches++;
-            if (fused) {
+            if (fused && geo.chunks == 1) {
                 if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
                 fused->deferred_splits = geo.splits + k_count;
                 fused->deferred_stride = geo.n_pad;
@@ -425,6 +448,11 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
             g.launches++;
         }
         if (g.profile && geo.chunks > 1) CUDA_TRY(cudaEventRecord(e1, st));
+        if (fused) {
+            fused->deferred_splits = 0;
+            fused->deferred_stride = n;
+            return COLATUS_OK;
+        }
     } else {
         const bool single = geo.splits == 1;
         float4 *fout = single ? out : partials;
@@ -605,7 +633,7 @@ int enqueue_step_table(cudaStream_t st) {
 // for the whole run (a captured graph keeps replaying the same value).
 int enqueue_run_head(cudaStream_t st, int generation) {
     const Workspace w = workspace_layout(g.n);
-    const Geometry geo = choose_geometry(g.n, g.n, false, true);
+    const Geometry geo = choose_geometry(g.n, g.n);
     const StepCoef *table = reinterpret_cast<const StepCoef *>(g.ws + w.step_table);
     int *ctr = reinterpret_cast<int *>(g.ws + w.step_ctr);
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);

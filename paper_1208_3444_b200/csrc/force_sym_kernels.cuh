@@ -40,13 +40,25 @@ __device__ __forceinline__ void sym_tile_body(const unsigned char *tile, const u
                                               const u64 (&nz)[IP], const u64 (&mi)[IP], u64 eps2_2, u64 (&ax)[IP],
                                               u64 (&ay)[IP], u64 (&az)[IP], float *racc, int lane) {
     const int f = (lane >> 2) & 7;
+    // Position p reads source p ^ f of the 128-byte row of 8 sources.  Two ways to form the address, measured on the
+    // B200 (N = 2^20, % of peak by the 20-flop convention): eight per-lane byte offsets (p ^ f) * 16 kept in registers
+    // (equal-mass body: 104.4 against 102.8), or the lane's row pointer plus a per-bit signed offset -- p ^ f =
+    // f + sum over the set bits b of p of (f has b ? -b : +b) -- which needs no extra registers (general body:
+    // 94.2 against 91.5); the first formulation, ((jb + p) ^ f) << 4 computed per load, gave 92.9 / 101.4.
+    int q[8];
+    if (EQM) {
+#pragma unroll
+        for (int p = 0; p < 8; ++p) q[p] = (p << 4) ^ (f << 4);
+    }
     for (int jb = 0; jb < TJ; jb += 8) {
         float vx[8], vy[8], vz[8];
+        const unsigned char *row = tile + (jb << 4) + (f << 4);   // this lane's source at position 0
 #pragma unroll
         for (int p = 0; p < 8; ++p) {
-            // (p ^ f) * 16 == (p * 16) ^ (f * 16); tile rows of 8 sources are 128-byte aligned
-            const float4 S = *reinterpret_cast<const float4 *>(
-                tile + (((jb + p) << 4) ^ (f << 4)));
+            const int off = ((p & 1) ? ((f & 1) ? -16 : 16) : 0) + ((p & 2) ? ((f & 2) ? -32 : 32) : 0) +
+                            ((p & 4) ? ((f & 4) ? -64 : 64) : 0);
+            const float4 S = EQM ? *reinterpret_cast<const float4 *>(tile + (jb << 4) + q[p])
+                                 : *reinterpret_cast<const float4 *>(row + off);
             const u64 X = pack2(S.x, S.x), Y = pack2(S.y, S.y), Z = pack2(S.z, S.z), M = pack2(S.w, S.w);
             u64 rx = 0ull, ry = 0ull, rz = 0ull;
 #pragma unroll
@@ -64,11 +76,11 @@ __device__ __forceinline__ void sym_tile_body(const unsigned char *tile, const u
                 const u64 r3 = mul2(rinv, rinv2);
                 const u64 wi = EQM ? r3 : mul2(r3, M);
                 const u64 wj = EQM ? r3 : mul2(r3, mi[i]);
-                ax[i] = fma2(wi, dx, ax[i]);
-                rx = fma2(wj, dx, rx);
-                ry = fma2(wj, dy, ry);
+ax[i] = fma2(wi, dx, ax[i]);
                 ay[i] = fma2(wi, dy, ay[i]);
                 az[i] = fma2(wi, dz, az[i]);
+                rx = fma2(wj, dx, rx);
+                ry = fma2(wj, dy, ry);
                 rz = fma2(wj, dz, rz);
             }
             float lo, hi;
@@ -146,7 +158,11 @@ __device__ __forceinline__ SymTile sym_tile_at(int p, int a, int nb, int k_begin
 // P = TPB * (k_count + (with_plain ? 1 + (NB even) : 0)) tiles.  Output rows of `stride` float4: row s =
 // target-side sums of split s (all NB * BT targets); row S + (k - k_begin) = reaction sums (already negated) of
 // block distance k.  Every row is written in full by every launch.
-template <int IP, int TJ, int NST, int MINB>
+// BODY: 0 = both tile bodies in the kernel, picked by the equal-mass flag; 1 = general body only, 2 = equal-mass
+// body only -- such a kernel returns at once when the flag asks for the other body, so launching the pair (1, 2) is
+// the same evaluation with each body scheduled by ptxas on its own (the two bodies in one kernel cost each other
+// 1-2.5 %); worth the second, empty launch for large problems only.
+template <int IP, int TJ, int NST, int MINB, int BODY>
 __global__ void __launch_bounds__(FORCE_THREADS, MINB)
 force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_begin, int k_count, int with_plain,
                  float eps2, float4 *__restrict__ partial, int64_t stride, const int *__restrict__ mass_flag,
@@ -164,6 +180,10 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int a = blockIdx.x, s = blockIdx.y;
+    if (BODY != 0) {                 // uniform over the grid; before any barrier or copy is set up
+        griddep_wait();
+        if ((__ldg(mass_flag) != generation) != (BODY == 2)) return;
+    }
     const int P = TPB * (k_count + (with_plain ? ((nb & 1) ? 1 : 2) : 0));
     const int p0 = (int)(((int64_t)s * P) / splits), p1 = (int)(((int64_t)(s + 1) * P) / splits);
     const unsigned char *src = reinterpret_cast<const unsigned char *>(staged);
@@ -222,12 +242,12 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
         for (int i = 0; i < IP; ++i) ax[i] = ay[i] = az[i] = ap[i] = 0ull;
         if (T.k == 0) {
             const float4 *tp = reinterpret_cast<const float4 *>(tile);
-            if (eqm)
+            if (BODY == 2 || (BODY == 0 && eqm))
                 force_tile_body<IP, TJ, false, true>(tp, nx, ny, nz, eps2_2, ax, ay, az, ap);
             else
                 force_tile_body<IP, TJ, false, false>(tp, nx, ny, nz, eps2_2, ax, ay, az, ap);
         } else {
-            if (eqm)
+            if (BODY == 2 || (BODY == 0 && eqm))
                 sym_tile_body<IP, TJ, true>(tile, nx, ny, nz, mi, eps2_2, ax, ay, az, racc, lane);
             else
                 sym_tile_body<IP, TJ, false>(tile, nx, ny, nz, mi, eps2_2, ax, ay, az, racc, lane);

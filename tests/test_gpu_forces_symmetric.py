@@ -1,6 +1,6 @@
 """The symmetric force kernel (every pair once, Newton's third law; force_sym_kernels.cuh, colatus_force_plan)
 against the FP64 oracle, through the C ABI.  It is picked automatically for whole-range evaluations of at least
-49152 bodies (configs 3-5: covered at full size in test_gpu_forces.py); here it is forced on at small and ragged
+24576 bodies (configs 2-5: covered at full size in test_gpu_forces.py); here it is forced on at small and ragged
 sizes so that every structural case is hit: 1 block (diagonal only), 2 blocks (antipodal only), odd and even
 block counts, ragged last blocks, every split count, equal and general masses, chunked evaluations.
 Tolerances: north_star's (G17), as in test_gpu_forces.py."""
@@ -181,12 +181,47 @@ def test_symmetric_steps_match_the_oracle_and_the_run_loop(session, symmetric_al
             assert np.array_equal(pos_a, pos_b) and np.array_equal(vel_a, vel_b), use_graph
 
 
+def test_symmetric_chunked_steps(session, symmetric_always):
+    """Steps whose force evaluation takes several launches of the symmetric kernel (partial rows capped): the kick
+    reads the accumulated forces; colatus_run (graphs, plain launches) == colatus_step loop bit for bit, and the
+    trajectory agrees with the single-launch one to rounding."""
+    n = 13000                                                        # 9 blocks, H = 4
+    pm = _problem(n, True, seed=3)
+    vel = np.zeros_like(pm)
+    eps2 = np.float32(1e-4)
+    steps, tau = 5, 1e-3
+    s = session
+    results = {}
+    for rows in (0, 6):                                              # automatic (1 launch) / 4 + 2 rows (2 launches)
+        B.colatus_set_option("source_splits", 4)
+        B.colatus_set_option("symmetric_rows", rows)
+        assert B.colatus_force_plan(n)["launches"] == (1 if rows == 0 else 2)
+        s.upload(pm, vel, eps2)
+        s.trace(np.arange(0, n, n // 16, dtype=np.int32)[:16], steps)
+        s.run(None, 1.0, tau, steps)
+        pos_a, vel_a = s.download()
+        tr_a = s.trace_read(0, steps)
+        for use_graph in (False, True):
+            s.upload(pm, vel, eps2)
+            s.trace(np.arange(0, n, n // 16, dtype=np.int32)[:16], steps)
+            s.run_native(None, 1.0, tau, steps, use_graph=use_graph)
+            pos_b, vel_b = s.download()
+            assert np.array_equal(pos_a, pos_b) and np.array_equal(vel_a, vel_b), (rows, use_graph)
+            assert np.array_equal(tr_a, s.trace_read(0, steps))
+        results[rows] = (pos_a, vel_a)
+    assert np.abs(results[0][0][:, :3] - results[6][0][:, :3]).max() < 1e-6
+    st = oracle.State(pm, vel, eps2, 1.0)
+    for _ in range(steps):
+        st.step(tau, 1.0, 0.0)
+    assert float(np.linalg.norm(results[6][0][:, :3].astype(np.float64) - st.x, axis=1).max()) <= 1e-5
+
+
 def test_plan_of_the_baseline_configurations(session):
     """What colatus_force_plan reports for BASELINE.json's sizes on this device."""
     if True:
-        small = B.colatus_force_plan(32768)
+        small = B.colatus_force_plan(4096)
         assert small["symmetric"] == 0
-        for n in (131072, 1 << 20):
+        for n in (32768, 131072, 1 << 20):
             p = B.colatus_force_plan(n)
             assert p["symmetric"] == 1 and p["launches"] == 1 and p["blocks"] == (n + 1535) // 1536
             assert p["partial_rows"] == p["splits"] + p["distances"]

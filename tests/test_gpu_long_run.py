@@ -10,8 +10,9 @@ runs per configuration: "A" from the inputs of record and "B" from inputs moved 
 the dynamics make of a perturbation below FP32 resolution, so it calibrates every threshold here; none is
 hand-picked after looking at a GPU result:
 
-    tol(statistic, checkpoint) = clip(100 * |A - B| / |A|,  1e-3,  min(3 * sat, 10 %))
     sat(statistic)             = max of |A - B| / |A| over the chaotic checkpoints (config 2: step >= 200)
+    tol(statistic, checkpoint) = clip(100 * |A - B| / |A|,  1e-3,  min(3 * sat, 10 %))     before chaos has saturated
+                               = min(3 * sat, 10 %)                                        at the chaotic checkpoints
 
 * 1e-3 floor: while the flow is laminar (config 2 up to the first collapse near step 50, all of config 3) A and
   B agree to 1e-5..1e-9 and the FP32 run is held to 1e-3 -- ten times tighter than G20's "within 1 %";
@@ -19,7 +20,13 @@ hand-picked after looking at a GPU result:
   does while the difference still grows;
 * 3 * sat: once chaos has saturated, GPU-vs-A is a draw from the same distribution as B-vs-A, whose largest
   value over ten checkpoints is `sat` (config 2 at 32^3: T 1.9 %, W 1.1 %, r_half 2.0 %, speed quantiles 1.6 %);
-  never looser than G20's 10 %.
+  never looser than G20's 10 %.  At a chaotic checkpoint the scale is `sat`, a property of the regime -- NOT the
+  pointwise |A - B| of that checkpoint, which is one draw and can be anywhere below it: the two oracle runs happen
+  to cross in W at step 800 (|A - B| / |A| = 1.0e-4 between checkpoints at 1e-2), so 100 x the pointwise value
+  would hold a third rounding realisation to 1.03 % there, below the 1.1 % the oracle's own runs differ by
+  elsewhere (tests/test_long_run_calibration.py asserts this spread from the committed JSON).  Every kernel the
+  library can take for this run -- the one-directional and the symmetric force kernel, two different summation
+  orders, i.e. two rounding realisations -- is run against the same thresholds.
 
 The 64-tracer speed percentiles of SURVEY G20 ("median and 90th percentile within 10 %") cannot be held to a
 relative bar: between the two ORACLE runs they differ by up to 17 % (median) and 21 % (p90) -- 64 samples of a
@@ -72,7 +79,8 @@ def calibrated_tolerances(block, chaotic_from):
     for k, sd in self_diff.items():
         chaotic = [d for a, d in zip(A, sd) if chaotic_from is not None and a["step"] >= chaotic_from]
         cap = min(3.0 * max(chaotic), CAP) if chaotic else CAP
-        tol[k] = [min(max(FACTOR * d, FLOOR), max(cap, FLOOR)) for d in sd]
+        tol[k] = [max(cap, FLOOR) if (chaotic_from is not None and a["step"] >= chaotic_from)
+                  else min(max(FACTOR * d, FLOOR), max(cap, FLOOR)) for a, d in zip(A, sd)]
     return tol, self_diff
 
 
@@ -81,7 +89,9 @@ def _parent_percentile(value, rec):
     return float(np.interp(value, rec["speed_q"], G.QUANTILES))
 
 
-def test_config2_full_size_1000_steps_statistics():
+@pytest.mark.parametrize("kernel", ["symmetric", "one-directional"])
+def test_config2_full_size_1000_steps_statistics(kernel):
+    from paper_1208_3444_b200 import binding as B
     from paper_1208_3444_b200.harness import Session
     gold = GOLD["config2"]
     A = gold["A"]
@@ -93,6 +103,8 @@ def test_config2_full_size_1000_steps_statistics():
 
     gpu = []
     with Session(cfg.G, cfg.n) as s:
+        B.colatus_set_option("symmetric", 1 if kernel == "symmetric" else 0)     # automatic choice / never
+        assert B.colatus_force_plan(cfg.n)["symmetric"] == (1 if kernel == "symmetric" else 0)
         s.upload(pm, vel, eps2)
         s.trace(tr_idx, 1000)
         a, done = cfg.a_start, 0
@@ -126,7 +138,7 @@ def test_config2_full_size_1000_steps_statistics():
                 at_ref = _parent_percentile(np.percentile(ts_ref, q), r)
                 worst[f"tracer_q{q}_points"] = max(worst.get(f"tracer_q{q}_points", 0.0), abs(at_gpu - at_ref))
                 assert abs(at_gpu - at_ref) <= 4.0 * np.sqrt(2.0) * sigma_pts, (r["step"], q, at_gpu, at_ref)
-    record_parity("1000-step config 2 at 32^3 vs golden oracle run", **worst)
+    record_parity(f"1000-step config 2 at 32^3 vs golden oracle run ({kernel} kernel)", **worst)
 
     # the run is not trivial: the box collapses onto its centre (G7) and the kinetic energy grows several-fold
     assert min(g["r_half"] for g in gpu) < 0.1 * gpu[0]["r_half"] and max(g["T"] for g in gpu) > 3 * gpu[0]["T"]

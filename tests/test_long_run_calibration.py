@@ -70,6 +70,13 @@ def test_one_ulp_sensitivity_at_full_size_is_what_the_docs_quote():
     assert 0.015 < sat["T"] < 0.025 and 0.008 < sat["W"] < 0.015 and 0.015 < sat["r_half"] < 0.025
     assert 0.010 < sat["q50"] < 0.020 and 0.010 < sat["q90"] < 0.020
     assert all(3 * v < 0.10 for v in sat.values())
+    # ... and inside that regime the pointwise |A - B| of ONE checkpoint is no scale: it is a single draw, and the two
+    # runs can cross -- W at step 800 differs by 1.0e-4 between neighbours at 1e-2, T spans a factor 5, r_half 7.
+    # The GPU test therefore holds every chaotic checkpoint to 3 x sat, not to 100 x its own pointwise difference
+    # (which at such a crossing, 1.03 % for W, would be tighter than what the oracle's two runs differ by elsewhere)
+    assert W[800] < 2e-4 and min(W[700], W[900]) > 50 * W[800] and 100 * W[800] < sat["W"]
+    for d in (T, W, R, q50):
+        assert max(d[s] for s in chaotic) > 4 * min(d[s] for s in chaotic)
     # the 64-tracer percentiles of SURVEY G20: the oracle differs from itself by far more than 10 %
     tm = _self_differences(c2, lambda r: float(np.median(r["tracer_speed"])))
     tp = _self_differences(c2, lambda r: float(np.percentile(r["tracer_speed"], 90)))
