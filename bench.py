@@ -42,7 +42,8 @@ FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.
 # summarised in profiles/: valid only for the (n, source splits) it was captured at -- reported as null otherwise.
 FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8, "symmetric": 0,
                              "profile": "profiles/r02_force_kernel_ncu_full.txt"}
-SYM_KERNEL_DRAM_TRAFFIC = None             # filled from the ncu --set full capture of force_sym_kernel (profiles/)
+SYM_KERNEL_DRAM_TRAFFIC = {"bytes": 361063936 + 5896358000, "n": 1 << 20, "splits": 13,
+                           "profile": "profiles/r02_force_sym_kernel_ncu_full.txt"}
 # executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
 # (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention
 EXECUTED_FLOP_GENERAL, EXECUTED_FLOP_EQUAL_MASS = 19.0, 18.0
@@ -320,7 +321,8 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
         executed = SYM_EXECUTED_FLOP_EQUAL_MASS if equal_mass else SYM_EXECUTED_FLOP_GENERAL
         # staged bodies read as targets and as sources, every partial row written once
         algorithmic_bytes = 16 * plan["padded_bodies"] * (2 + plan["splits"] + plan["distances"])
-        kernel = "force_sym_kernel<3,512,4,2> (every pair once, applied to both bodies)%s%s" % (
+        kernel = "force_sym_kernel<3,512,4,2,%s> (every pair once, applied to both bodies)%s%s" % (
+            ("2" if equal_mass else "1") if plan["padded_bodies"] >= 98304 else "0",
             " equal-mass loop" if equal_mass else "",
             "; %d launches + partial-row reductions per evaluation" % plan["launches"] if plan["launches"] > 1 else "")
     else:
