@@ -321,7 +321,8 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
         executed = SYM_EXECUTED_FLOP_EQUAL_MASS if equal_mass else SYM_EXECUTED_FLOP_GENERAL
         # staged bodies read as targets and as sources, every partial row written once
         algorithmic_bytes = 16 * plan["padded_bodies"] * (2 + plan["splits"] + plan["distances"])
-        kernel = "force_sym_kernel<3,512,4,2,%s> (every pair once, applied to both bodies)%s%s" % (
+        kernel = "force_sym_kernel<%d,%d,4,2,%s> (every pair once, applied to both bodies)%s%s" % (
+            geo["targets_per_thread"] // 2, 512 if geo["targets_per_thread"] == 6 else 256,
             ("2" if equal_mass else "1") if plan["padded_bodies"] >= 98304 else "0",
             " equal-mass loop" if equal_mass else "",
             "; %d launches + partial-row reductions per evaluation" % plan["launches"] if plan["launches"] > 1 else "")

@@ -290,10 +290,10 @@ int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
  * Whole-range evaluations (target_count == n) without the potential and with at least 24576 bodies use the
  * SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
  * per unordered pair and applied to both bodies (Newton's third law) -- 16 packed FP32 operations per
- * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 1536; block a meets the `distances`
+ * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 1536 (1024 below 65536 bodies); block a meets the `distances`
  * blocks a+1 .. a+distances (mod blocks) both ways, and itself (and the antipodal block when `blocks` is even)
  * one way.  The sums a block receives from each distance are kept as partial rows in the workspace and
- * added in fixed row order (in FP64 when there are more than 64 rows), so results are reproducible bit for
+ * added in fixed row order (in FP64 when there are more than 16 rows), so results are reproducible bit for
  * bit; when the rows of all distances exceed 8 GiB the evaluation runs as `launches` kernel launches of
  * `distances_per_launch` distances each.  Target sub-ranges, potential evaluations and smaller problems take
  * the one-directional kernel (out[0] = 0; its geometry is colatus_force_geometry's).
@@ -307,6 +307,8 @@ int colatus_force_plan(int64_t n, int64_t target_count, int with_potential, int6
  *   "source_splits" in [0,64] (capped at 16 above 65536 bodies and for the symmetric kernel);
  *   "symmetric": 0 = never use the symmetric kernel, 1 = automatic (default after colatus_init),
  *                2 = whenever the evaluation allows it (any n; for tests);
+ *   "symmetric_block": bodies per block of the symmetric kernel, 1024 or 1536 (0 = automatic: 1024 below 65536
+ *                bodies, 1536 from there on);
  *   "symmetric_rows": cap on the partial rows one launch of the symmetric kernel may use (0 = what the
  *                workspace holds, else >= 2): a small value splits an evaluation into several launches. */
 int colatus_set_option(const char *name, int64_t value);

@@ -31,9 +31,10 @@ constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in c
 constexpr int GRAPH_STEPS = 8;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
 
 // symmetric (each pair once) force kernel, force_sym_kernels.cuh: whole-range evaluations of at least SYM_MIN_N bodies
-constexpr int SYM_IP = 3, SYM_TJ = 512;
-constexpr int64_t SYM_BT = (int64_t)FORCE_THREADS * 2 * SYM_IP;   // bodies per block = targets of one CTA
-constexpr int SYM_TPB = (int)(SYM_BT / SYM_TJ);                   // tiles per block
+// Two variants: blocks of 1536 bodies (6 targets per thread, 512-source tiles) and, below SYM_MID_N bodies, blocks of
+// 1024 (4 targets per thread, 256-source tiles), whose finer tiles split better over the SMs (N = 32768: 32 x 14
+// CTAs of 4.9 tiles against 22 x 13 of 2.8; 7 % faster; profiles/r02_symmetric_kernel.md section 4b)
+constexpr int64_t SYM_MID_N = 65536;
 constexpr int64_t SYM_MIN_N = 24576;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
 constexpr int SYM_MAX_SPLITS = 16;
 constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)
@@ -49,6 +50,8 @@ struct Geometry {
     // K of them per launch (K reaction rows + `splits` target-side rows in the workspace), `chunks` launches
     bool sym = false;
     int nb = 0, H = 0, K = 0, chunks = 0;
+    int64_t bt() const { return (int64_t)FORCE_THREADS * 2 * IP; }   // bodies per block = targets of one CTA
+    int tpb() const { return (int)(bt() / TJ); }                      // tiles per block
 };
 
 struct Workspace {     // byte offsets inside the caller's workspace
@@ -81,6 +84,7 @@ struct Context {
     int64_t launches = 0;
     // tuning overrides (0 = automatic)
     int force_I = 0, force_splits = 0;
+    int sym_block = 0;    // 0 = automatic, else 1024 or 1536 bodies per block ("symmetric_block")
     int sym_rows = 0;     // cap on partial rows per launch of the symmetric kernel (0 = what the workspace holds)
     int symmetric = 1;    // 0 = never, 1 = automatic (n >= SYM_MIN_N), 2 = whenever the evaluation allows it
     int init_epoch = 0;   // counts colatus_init calls
@@ -142,19 +146,28 @@ inline int max_splits(int64_t n) { return n <= SMALL_N ? MAX_SPLITS : MAX_SPLITS
 // rows of force_sym_kernel -- all of them ((splits + H) rows of n_pad bodies) while that stays within
 // SYM_ROWS_BUDGET, else the budget (the evaluation is then chunked over block distances), never fewer than
 // SYM_MAX_SPLITS + SYM_MIN_ROWS rows.  Non-decreasing in n, so a workspace sized for n_max serves every n <= n_max.
-inline int64_t sym_blocks(int64_t n) { return (n + SYM_BT - 1) / SYM_BT; }
-size_t partials_bytes(int64_t n) {
-    size_t bytes = (size_t)max_splits(n) * (size_t)n * 16;
-    const size_t row = (size_t)sym_blocks(n) * SYM_BT * 16;
-    if (bytes < (SYM_MAX_SPLITS + 2) * row) bytes = (SYM_MAX_SPLITS + 2) * row;   // tiny n with "symmetric" = 2
+inline int sym_ip(int64_t n) { return g.sym_block ? g.sym_block / 512 : (n < SYM_MID_N ? 2 : 3); }
+inline int64_t sym_blocks(int64_t n, int ip) { return (n + 512 * ip - 1) / (512 * ip); }
+size_t sym_rows_bytes(int64_t n, int ip) {
+    const size_t row = (size_t)sym_blocks(n, ip) * 512 * ip * 16;
+    size_t bytes = (SYM_MAX_SPLITS + 2) * row;                      // tiny n with "symmetric" = 2
     if (n >= SYM_MIN_N) {
-        const size_t H = (size_t)((sym_blocks(n) - 1) / 2);
+        const size_t H = (size_t)((sym_blocks(n, ip) - 1) / 2);
         size_t want = (SYM_MAX_SPLITS + H) * row;
         if (want > SYM_ROWS_BUDGET) want = SYM_ROWS_BUDGET;
         const size_t least = (size_t)(SYM_MAX_SPLITS + SYM_MIN_ROWS) * row;
         if (want < least) want = least;
         if (want > bytes) bytes = want;
     }
+    return bytes;
+}
+// The 1536-body variant's need at n and the 1024-body variant's at min(n, SYM_MID_N - 1) (it is the automatic choice
+// only below SYM_MID_N; forced above, it gets by with what is there -- more launches): non-decreasing across SYM_MID_N.
+size_t partials_bytes(int64_t n) {
+    size_t bytes = (size_t)max_splits(n) * (size_t)n * 16;
+    if (sym_rows_bytes(n, 3) > bytes) bytes = sym_rows_bytes(n, 3);
+    const int64_t n_mid = n < SYM_MID_N ? n : SYM_MID_N - 1;
+    if (sym_rows_bytes(n_mid, 2) > bytes) bytes = sym_rows_bytes(n_mid, 2);
     return bytes;
 }
 
@@ -237,11 +250,11 @@ bool sym_eligible(int64_t n, int64_t t_count, bool potential) {
 Geometry choose_sym_geometry(int64_t n) {
     Geometry geo;
     geo.sym = true;
-    geo.IP = SYM_IP;
-    geo.TJ = SYM_TJ;
-    geo.nb = (int)sym_blocks(n);
+    geo.IP = sym_ip(n);
+    geo.TJ = geo.IP == 3 ? 512 : 256;
+    geo.nb = (int)sym_blocks(n, geo.IP);
     geo.tiles_t = geo.nb;
-    geo.n_pad = (int64_t)geo.nb * SYM_BT;
+    geo.n_pad = (int64_t)geo.nb * geo.bt();
     geo.H = (geo.nb - 1) / 2;
     int64_t rows_avail = (int64_t)(partials_bytes(n) / ((size_t)geo.n_pad * 16));
     if (g.sym_rows >= 2 && g.sym_rows < rows_avail) rows_avail = g.sym_rows;   // "symmetric_rows": forces chunking
@@ -249,7 +262,9 @@ Geometry choose_sym_geometry(int64_t n) {
         geo.sym = false;
         return geo;
     }
-    const double plain_tiles = SYM_TPB * ((geo.nb & 1) ? 1.0 : 2.0) * 0.68;   // a one-directional tile costs ~0.68 symmetric ones
+    const int tpb = geo.tpb();
+    const double plain_tiles = tpb * ((geo.nb & 1) ? 1.0 : 2.0) * 0.68;   // a one-directional tile costs ~0.68 symmetric ones
+    const double c0 = geo.IP == 3 ? 0.04 : 0.12;                           // per-CTA overhead in units of one tile
     double best_cost = -1.0;
     for (int s = 1; s <= SYM_MAX_SPLITS; ++s) {
         if (g.force_splits && g.force_splits <= SYM_MAX_SPLITS && g.force_splits < rows_avail && s != g.force_splits)
@@ -260,8 +275,8 @@ Geometry choose_sym_geometry(int64_t n) {
         if (K < 1) K = 1;
         const int chunks = geo.H == 0 ? 1 : (geo.H + K - 1) / K;
         const double per_sm = (double)(((int64_t)geo.nb * s + g.sm_count - 1) / g.sm_count);
-        const double tiles = (plain_tiles + (double)SYM_TPB * geo.H) / s;
-        const double cost = tiles * (per_sm + 0.096) + chunks * per_sm * 0.04;
+        const double tiles = (plain_tiles + (double)tpb * geo.H) / s;
+        const double cost = tiles * (per_sm + 0.096) + chunks * per_sm * c0;
         if (best_cost < 0.0 || cost < best_cost * 0.998) {
             best_cost = cost;
             geo.splits = s;
@@ -269,7 +284,7 @@ Geometry choose_sym_geometry(int64_t n) {
             geo.chunks = chunks;
         }
     }
-    geo.tiles_per_split = (int)((SYM_TPB * (geo.H + 2) + geo.splits - 1) / geo.splits);
+    geo.tiles_per_split = (int)((tpb * (geo.H + 2) + geo.splits - 1) / geo.splits);
     return geo;
 }
 
@@ -285,12 +300,12 @@ Geometry choose_geometry(int64_t n, int64_t t_count, bool potential = false) {
 // device), or -- from SYM_PAIR_N bodies on -- two launches, a general-only and an equal-mass-only kernel, of which the
 // one the equal-mass flag does not ask for returns at once (15 us at 2^20): compiled alone the general body runs
 // 2.4 % faster (94.0 % against 91.8 % of peak at 2^20; the equal-mass body is the same either way).
-template <int BODY>
+template <int IP, int TJ, int BODY>
 cudaError_t launch_force_sym_body(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
                                   float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
                                   cudaStream_t st, bool pdl) {
-    auto kern = force_sym_kernel<SYM_IP, SYM_TJ, NSTAGES, 2, BODY>;
-    const size_t smem = force_sym_smem_bytes<SYM_IP, SYM_TJ, NSTAGES>();
+    auto kern = force_sym_kernel<IP, TJ, NSTAGES, 2, BODY>;
+    const size_t smem = force_sym_smem_bytes<IP, TJ, NSTAGES>();
     static int attr_epoch = 0;
     if (attr_epoch != g.init_epoch) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -307,15 +322,18 @@ inline bool sym_pair(const Geometry &geo) { return geo.n_pad >= SYM_PAIR_N; }
 cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
                              float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
                              cudaStream_t st, bool pdl) {
+    if (geo.IP == 2)
+        return launch_force_sym_body<2, 256, 0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
+                                                generation, step_ctr, st, pdl);
     if (!sym_pair(geo))
-        return launch_force_sym_body<0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
-                                        generation, step_ctr, st, pdl);
-    cudaError_t e = launch_force_sym_body<1>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
-                                             generation, step_ctr, st, pdl);
+        return launch_force_sym_body<3, 512, 0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
+                                                generation, step_ctr, st, pdl);
+    cudaError_t e = launch_force_sym_body<3, 512, 1>(geo, packed, k_begin, k_count, with_plain, eps2, partials,
+                                                     mass_flag, generation, step_ctr, st, pdl);
     if (e != cudaSuccess) return e;
     g.launches++;
-    return launch_force_sym_body<2>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag, generation,
-                                    step_ctr, st, pdl);
+    return launch_force_sym_body<3, 512, 2>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
+                                            generation, step_ctr, st, pdl);
 }
 
 template <int IP, int TJ, bool POT>
@@ -729,6 +747,7 @@ int colatus_init(const colatus_config *cfg) {
     g.force_I = g.force_splits = 0;
     g.symmetric = 1;
     g.sym_rows = 0;
+    g.sym_block = 0;
     g.def_S = g.bg_rho = 0.0;
     invalidate_graph();
     g.initialised = true;
@@ -1289,6 +1308,9 @@ int colatus_set_option(const char *name, int64_t value) {
     } else if (!strcmp(name, "symmetric")) {
         if (value < 0 || value > 2) return fail(COLATUS_INVALID_ARG, "must be 0 (never), 1 (automatic) or 2 (always)");
         g.symmetric = (int)value;
+    } else if (!strcmp(name, "symmetric_block")) {
+        if (value != 0 && value != 1024 && value != 1536) return fail(COLATUS_INVALID_ARG, "must be 0, 1024 or 1536");
+        g.sym_block = (int)value;
     } else if (!strcmp(name, "symmetric_rows")) {
         if (value < 0 || value == 1 || value > 1000000) return fail(COLATUS_INVALID_ARG, "must be 0 or >= 2");
         g.sym_rows = (int)value;

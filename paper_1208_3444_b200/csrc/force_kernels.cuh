@@ -324,15 +324,17 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
 
 constexpr int REDUCE_MAX_SPLITS = 64;   // upper bound on source splits (small problems; large ones use <= 16)
 constexpr int REDUCE_CHUNK = 16;        // partials loaded together (held in registers below)
+constexpr int REDUCE_WIDE_FROM = 17;    // rows from which sum_partials accumulates in FP64
 
 // Sum of the `splits` partials of target t in row order 0, 1, 2, ...: 16 loads at a time (independent, so
 // their latencies overlap), then the adds in fixed order -- the result does not depend on the chunking.
-// Up to REDUCE_MAX_SPLITS rows (the source splits of force_kernel) are added in FP32; more rows (the reaction
-// rows of force_sym_kernel: hundreds) are added in FP64 and rounded once, so the row count does not show in the
-// result's error.  A pure function of (rows, values): every caller gets the same bits.
+// Up to REDUCE_WIDE_FROM - 1 rows (the automatic source splits of force_kernel: <= 16) are added in FP32; more rows
+// (the reaction rows of force_sym_kernel: tens to hundreds; forced split counts) are added in FP64 and rounded
+// once, so the row count does not show in the result's error.  A pure function of (rows, values): every caller gets
+// the same bits.
 __device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partial, int64_t stride, int splits,
                                                int64_t t) {
-    if (splits > REDUCE_MAX_SPLITS) {
+    if (splits >= REDUCE_WIDE_FROM) {
         double sx = 0.0, sy = 0.0, sz = 0.0, sw = 0.0;
         for (int k0 = 0; k0 < splits; k0 += REDUCE_CHUNK) {
             float4 q[REDUCE_CHUNK];
