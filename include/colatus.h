@@ -83,8 +83,12 @@ typedef struct colatus_config {
 typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosmo;
 
 /* Bytes of device workspace needed for problems up to n_max bodies: the staged (padded)
- * source array, source-split partial sums, reduction scratch, and staging for the
- * host-buffer entry point.  Pure host arithmetic; 0 if n_max < 1. */
+ * source array, the partial-sum rows, reduction scratch, and staging for the host-buffer
+ * entry point.  From 24576 bodies on the partial rows are those of the symmetric force kernel
+ * (colatus_force_plan): one row of 16 bytes per body for every source split and every block
+ * distance, capped at 8 GiB -- 0.13 GB at n = 131072, 6.1 GB at 2^20, 8.9 GB at 2^22 (about
+ * 1.1 KB per body below 24576).  Non-decreasing in n_max: a workspace sized for n_max serves
+ * every n <= n_max.  Pure host arithmetic; 0 if n_max < 1. */
 size_t colatus_workspace_bytes(int64_t n_max);
 
 /* Selects the device, checks it is cc 10.x, records G and the workspace.  A second
@@ -99,6 +103,9 @@ void colatus_shutdown(void);
  *                branched around (reading G4): it is m_k eps2^-1.5 * 0 = 0 exactly, PROVIDED m_k eps2^-1.5 is
  *                finite in FP32 -- the caller keeps |m| * eps2^-1.5 < 3e38 (at the floor: |m| < 3e2), else
  *                that target's force is NaN.  The same bound keeps close distinct pairs finite.
+ * Whole-range evaluations of >= 24576 bodies evaluate every pair once and apply it to both bodies
+ * (the symmetric kernel, colatus_force_plan); results agree with the one-directional kernel to FP32
+ * summation rounding, and either is bitwise reproducible from run to run.
  * Enqueues on cuda_stream and returns without synchronising.  n in [1, 2^31-1];
  * pointers 16-byte aligned and distinct. */
 int colatus_forces(const void *pos_mass_dev, int64_t n, float eps2, void *acc_out_dev,
