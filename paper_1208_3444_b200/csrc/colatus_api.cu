@@ -28,7 +28,13 @@ constexpr int NSTAGES = 4;            // shared-memory ring depth
 constexpr int DIAG_BLOCKS_MAX = 1024;
 constexpr int64_t PAD_SOURCES = 1024; // n_pad granularity = largest tile
 constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in colatus_run
-constexpr int GRAPH_STEPS = 8;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
+#ifndef COLATUS_GRAPH_STEPS
+#define COLATUS_GRAPH_STEPS 8
+#endif
+#ifndef COLATUS_TAIL_THREADS
+#define COLATUS_TAIL_THREADS 256
+#endif
+constexpr int GRAPH_STEPS = COLATUS_GRAPH_STEPS;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
 
 // symmetric (each pair once) force kernel, force_sym_kernels.cuh: whole-range evaluations of at least SYM_MIN_N bodies
 // Two variants: blocks of 1536 bodies (6 targets per thread, 512-source tiles) and, below SYM_MID_N bodies, blocks of
@@ -675,18 +681,18 @@ int enqueue_step_two_kernels(cudaStream_t st, int generation) {
     f.pdl = true;
     int rc = run_forces(g.pos, g.n, 0, g.n, g.eps2, g.acc, false, st, &f);
     if (rc) return rc;
-    const unsigned blocks = (unsigned)((f.geo.n_pad + 255) / 256);
+    const unsigned blocks = (unsigned)((f.geo.n_pad + COLATUS_TAIL_THREADS - 1) / COLATUS_TAIL_THREADS);
     const int32_t *slot = reinterpret_cast<const int32_t *>(g.ws + w.trace_slot);
     const float4 *partials = reinterpret_cast<const float4 *>(g.ws + w.partials);
     float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
     int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
     cudaError_t e;
     if (g.trace_k > 0)
-        e = launch_ex(step_tail_head_kernel<true>, dim3(blocks), dim3(256), 0, st, true, g.pos, g.vel, g.acc, partials,
+        e = launch_ex(step_tail_head_kernel<true>, dim3(blocks), dim3(COLATUS_TAIL_THREADS), 0, st, true, g.pos, g.vel, g.acc, partials,
                       f.deferred_stride, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, slot, g.ring, g.trace_k, packed,
                       mass_flag, generation);
     else
-        e = launch_ex(step_tail_head_kernel<false>, dim3(blocks), dim3(256), 0, st, true, g.pos, g.vel, g.acc, partials,
+        e = launch_ex(step_tail_head_kernel<false>, dim3(blocks), dim3(COLATUS_TAIL_THREADS), 0, st, true, g.pos, g.vel, g.acc, partials,
                       f.deferred_stride, f.deferred_splits, g.n, f.geo.n_pad, (float)g.G, table, ctr, (const int32_t *)nullptr,
                       (float4 *)nullptr, 0, packed, mass_flag, generation);
     CUDA_TRY(e);

@@ -44,8 +44,18 @@ void dopri(const Deriv &F, double y[2], double dt) {
                         e6 = 22.0 / 525, e7 = -1.0 / 40;
     (void)c2; (void)c3; (void)c4; (void)c5;   // autonomous system: the nodes are not needed
     const double rtol = 1e-13;
-    double t = 0.0, h = dt / 16.0;
     const double dir = (dt >= 0) ? 1.0 : -1.0;
+    // first trial step: the whole interval, but no more than a tenth of the Hubble time at the start (the natural
+    // scale of eq. (2)); the controller below shrinks or grows it from there.  A leapfrog half step is << 1/H, so the
+    // per-step schedule of colatus_run costs one accepted step per call (it used to start at dt/16: 16 steps per
+    // call, 1.5 us per leapfrog step -- a tenth of a whole N = 4096 step spent on the host before the first launch)
+    double t = 0.0, h = dt;
+    {
+        double f0[2];
+        F(y, f0);
+        const double rate = std::fabs(f0[0]) / std::fmax(std::fabs(y[0]), 1e-300);      // |da/dt| / a = H
+        if (std::isfinite(rate) && rate > 0.0 && std::fabs(h) * rate > 0.1) h = dir * 0.1 / rate;
+    }
     double k1[2], k2[2], k3[2], k4[2], k5[2], k6[2], k7[2], w[2], ynew[2];
     int guard = 0;
     while ((dt - t) * dir > 0 && guard++ < 1000000) {
