@@ -14,9 +14,10 @@ colatus_diagnostics (momentum / kinetic energy reductions).  N^2 pair interactio
 --impl reference times the FP64 CPU oracle (oracle/) on the host cores on a bounded sample of the
 same workload; it is a deliberately slow baseline, not the target.
 
-N > 1 (one rank per GPU): eq. (1) sharded by targets, positions all-gathered over NCCL once per step after
-the first drift (the path's only exchange step), diagnostics by one all-reduce; total work fixed ->
-"scaling": "strong".  Under torchrun the ranks come from the environment; a plain `python bench.py --gpus N`
+N > 1 (one rank per GPU): bodies owned in slices, positions all-gathered over NCCL once per step after the first
+drift; eq. (1) divided by block pairs (symmetric evaluation: every rank evaluates its share of the unordered pairs,
+one all-reduce of the float4[n] partial forces) or, below 24576 bodies, by targets; diagnostics by one all-reduce;
+total work fixed -> "scaling": "strong".  Under torchrun the ranks come from the environment; a plain `python bench.py --gpus N`
 re-launches itself under torch.distributed.run with N ranks (and fails loudly if fewer GPUs are visible).
 """
 from __future__ import annotations
@@ -306,8 +307,9 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
 
     # ---- roofline of the dominant kernel (force kernel), from events inside the timed region
     pairs_per_launch = float(count) * n
-    geo = B.colatus_force_geometry(n, count)
-    plan = B.colatus_force_plan(n, count)
+    sharded_sym = stepper is not None and stepper.symmetric       # N > 1: every rank evaluates its share of the pairs
+    geo = B.colatus_force_geometry(n, n if sharded_sym else count)
+    plan = B.colatus_force_plan(n, n if sharded_sym else count)
     geo["plan"] = plan
     sym = bool(plan["symmetric"])
     equal_mass = bool(np.all(pm[:, 3] == pm[0, 3]))
@@ -326,6 +328,8 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
             ("2" if equal_mass else "1") if plan["padded_bodies"] >= 98304 else "0",
             " equal-mass loop" if equal_mass else "",
             "; %d launches + partial-row reductions per evaluation" % plan["launches"] if plan["launches"] > 1 else "")
+        if sharded_sym:
+            kernel += "; share %d of %d of the block pairs per rank, one all-reduce of the partial forces" % (rank, world)
     else:
         cap = FORCE_KERNEL_DRAM_TRAFFIC
         traffic = cap["bytes"] if (n == cap["n"] and world == 1 and geo["source_splits"] == cap["splits"]) else None
@@ -439,7 +443,9 @@ def run_native(args):
             "config": {"workload": f"config {cfg.index} ({cfg.name}): N={n}, " + WORKLOAD_TEXT[cfg.index] +
                                    f", eps={cfg.eps}; one full leapfrog step + diagnostics per step",
                        "n": n, "interactions_per_step": float(n) * n, "tracers": N_TRACERS,
-                       "parallelism": "single GPU" if world == 1 else f"targets sharded over {world} GPUs, "
+                       "parallelism": "single GPU" if world == 1 else f"eq. (1) divided over {world} GPUs (symmetric "
+                                                                       "evaluation: by block pairs, one all-reduce of "
+                                                                       "the partial forces per step; else by targets), "
                                                                        "one all-gather of positions per step, "
                                                                        "one all-reduce of 16 doubles for the diagnostics",
                        "l2_flush": "256 MiB memset between steps (inside the timed region)",

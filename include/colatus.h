@@ -122,6 +122,18 @@ int colatus_forces_potential(const void *pos_mass_dev, int64_t n, float eps2, vo
 int colatus_forces_range(const void *pos_mass_dev, int64_t n, int64_t target_begin,
                          int64_t target_count, float eps2, void *acc_out_dev, void *cuda_stream);
 
+/* One share of a SYMMETRIC evaluation of eq. (1) (colatus_force_plan): the block pairs whose target
+ * block lies in share `part` of `parts` -- contiguous ranges of the blocks, equal work because the pairing is
+ * circulant.  acc_out_dev = float4[n], ALL bodies: G x what those pairs deliver, to their own blocks and, as
+ * reactions (Newton's third law), to the blocks they meet; exactly 0 for bodies they do not reach.  The outputs of
+ * the shares 0 .. parts-1 add up to the whole force: this is how eq. (1) is divided over GPUs without giving up the
+ * single evaluation of every pair -- every GPU holds all positions (one all-gather per step, as for target sharding),
+ * evaluates share `rank` of `world`, and ONE all-reduce of the float4[n] outputs gives every GPU the forces
+ * (paper_1208_3444_b200/sharded.py).  Any n for which the workspace holds two partial rows (else INVALID_ARG).
+ * Same argument rules as colatus_forces; enqueues on cuda_stream. */
+int colatus_forces_symmetric_part(const void *pos_mass_dev, int64_t n, float eps2, int part, int parts,
+                                  void *acc_out_dev, void *cuda_stream);
+
 /* Host-buffer variant: copies float4[n] host -> device, evaluates eq. (1), copies
  * float4[n] back and synchronises.  Uses the workspace staging area and the stream given
  * (NULL = default).  This is the end-to-end call bench.py's "e2e" times. */
@@ -221,6 +233,11 @@ int colatus_drift(double d);
 /* Force on the resident state's target range into acc_dev, then the fused kick-drift
  * (eqs. (4)-(5)) v = cv v + ck F; x += d2 v and the tracer record.  Asynchronous. */
 int colatus_force_kick_drift(double cv, double ck, double d2);
+/* The kick-drift alone, with forces the caller supplies: acc_dev = const float4[target_count] (F of the target
+ * range's bodies, G applied, indexed from the range's first body) -> v = cv v + ck F; x += d2 v, tracer record,
+ * step counter + 1.  This is the second half of colatus_force_kick_drift for drivers that assemble F themselves
+ * (the sharded symmetric evaluation: colatus_forces_symmetric_part on every GPU, one all-reduce).  Asynchronous. */
+int colatus_kick_drift(const void *acc_dev, double cv, double ck, double d2);
 
 /* ---- tracers -------------------------------------------------
  * After each step the velocities v^{n+1} of the k particles idx_dev[0..k) are written to

@@ -61,6 +61,8 @@ SIGNATURES = {
     "colatus_set_target_range": (c_int, [c_int64, c_int64]),
     "colatus_drift": (c_int, [c_double]),
     "colatus_force_kick_drift": (c_int, [c_double, c_double, c_double]),
+    "colatus_kick_drift": (c_int, [c_void_p, c_double, c_double, c_double]),
+    "colatus_forces_symmetric_part": (c_int, [c_void_p, c_int64, c_float, c_int, c_int, c_void_p, c_void_p]),
     "colatus_trace": (c_int, [c_void_p, c_int, c_void_p, c_int]),
     "colatus_trace_read": (c_int, [c_void_p, c_int64, c_int]),
     "colatus_splat": (c_int, [c_void_p, c_int64, c_int, POINTER(c_float), c_int, c_int, c_void_p, c_void_p]),
@@ -165,6 +167,11 @@ def colatus_forces_range(pos_mass, n, target_begin, target_count, eps2, acc_out,
                                       _ptr(acc_out), _stream(stream)))
 
 
+def colatus_forces_symmetric_part(pos_mass, n, eps2, part, parts, acc_out, stream=None):
+    _check(lib().colatus_forces_symmetric_part(_ptr(pos_mass), int(n), float(eps2), int(part), int(parts),
+                                               _ptr(acc_out), _stream(stream)))
+
+
 def colatus_forces_host(pos_mass_host, n, eps2, acc_out_host, stream=None):
     """Host buffers: numpy float32 arrays or pinned torch CPU tensors of shape [n,4]."""
     _check(lib().colatus_forces_host(_host_ptr(pos_mass_host), int(n), float(eps2), _host_ptr(acc_out_host),
@@ -250,6 +257,10 @@ def colatus_drift(d):
 
 def colatus_force_kick_drift(cv, ck, d2):
     _check(lib().colatus_force_kick_drift(float(cv), float(ck), float(d2)))
+
+
+def colatus_kick_drift(acc, cv, ck, d2):
+    _check(lib().colatus_kick_drift(_ptr(acc), float(cv), float(ck), float(d2)))
 
 
 def colatus_trace(idx, k, ring, capacity_steps):

@@ -56,6 +56,7 @@ struct Geometry {
     // K of them per launch (K reaction rows + `splits` target-side rows in the workspace), `chunks` launches
     bool sym = false;
     int nb = 0, H = 0, K = 0, chunks = 0;
+    int a_begin = 0, a_count = 0;   // target blocks of this evaluation (all nb of them unless it is a share: ..._part)
     int64_t bt() const { return (int64_t)FORCE_THREADS * 2 * IP; }   // bodies per block = targets of one CTA
     int tpb() const { return (int)(bt() / TJ); }                      // tiles per block
 };
@@ -253,12 +254,14 @@ bool sym_eligible(int64_t n, int64_t t_count, bool potential) {
     return g.symmetric == 2 || n >= SYM_MIN_N;
 }
 
-Geometry choose_sym_geometry(int64_t n) {
+Geometry choose_sym_geometry(int64_t n, int part = 0, int parts = 1) {
     Geometry geo;
     geo.sym = true;
     geo.IP = sym_ip(n);
     geo.TJ = geo.IP == 3 ? 512 : 256;
     geo.nb = (int)sym_blocks(n, geo.IP);
+    geo.a_begin = (int)((int64_t)geo.nb * part / parts);
+    geo.a_count = (int)((int64_t)geo.nb * (part + 1) / parts) - geo.a_begin;
     geo.tiles_t = geo.nb;
     geo.n_pad = (int64_t)geo.nb * geo.bt();
     geo.H = (geo.nb - 1) / 2;
@@ -280,7 +283,8 @@ Geometry choose_sym_geometry(int64_t n) {
         if (K > geo.H) K = geo.H;
         if (K < 1) K = 1;
         const int chunks = geo.H == 0 ? 1 : (geo.H + K - 1) / K;
-        const double per_sm = (double)(((int64_t)geo.nb * s + g.sm_count - 1) / g.sm_count);
+        const int64_t ctas = (int64_t)(geo.a_count > 0 ? geo.a_count : 1) * s;
+        const double per_sm = (double)((ctas + g.sm_count - 1) / g.sm_count);
         const double tiles = (plain_tiles + (double)tpb * geo.H) / s;
         const double cost = tiles * (per_sm + 0.096) + chunks * per_sm * c0;
         if (best_cost < 0.0 || cost < best_cost * 0.998) {
@@ -318,9 +322,9 @@ cudaError_t launch_force_sym_body(const Geometry &geo, const float4 *packed, int
         if (e != cudaSuccess) return e;
         attr_epoch = g.init_epoch;
     }
-    dim3 grid((unsigned)geo.nb, (unsigned)geo.splits);
-    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, packed, geo.nb, geo.splits, k_begin, k_count,
-                     with_plain, eps2, partials, geo.n_pad, mass_flag, generation, step_ctr);
+    dim3 grid((unsigned)geo.a_count, (unsigned)geo.splits);
+    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, packed, geo.nb, geo.a_begin, geo.splits, k_begin,
+                     k_count, with_plain, eps2, partials, geo.n_pad, mass_flag, generation, step_ctr);
 }
 
 inline bool sym_pair(const Geometry &geo) { return geo.n_pad >= SYM_PAIR_N; }
@@ -518,6 +522,67 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
     return COLATUS_OK;
 }
 
+// One share of a symmetric evaluation: the block pairs whose target block lies in share `part` of `parts` (contiguous
+// block ranges of near-equal length: equal work, the pairing is circulant).  out[n] = G x what those pairs deliver, to
+// their target blocks and, as reactions, to the blocks they meet -- 0 where they deliver nothing.  The outputs of all
+// shares add up to the whole force.
+int run_forces_sym_part(const float4 *pos_mass, int64_t n, float eps2, int part, int parts, float4 *out,
+                        cudaStream_t st) {
+    const Workspace w = workspace_layout(n);
+    if (w.total > g.ws_bytes)
+        return fail(COLATUS_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, n=%lld needs %zu", g.ws_bytes,
+                    (long long)n, w.total);
+    const Geometry geo = choose_sym_geometry(n, part, parts);
+    if (!geo.sym) return fail(COLATUS_INVALID_ARG, "n=%lld is too small for a symmetric evaluation", (long long)n);
+    float4 *packed = reinterpret_cast<float4 *>(g.ws + w.packed);
+    float4 *partials = reinterpret_cast<float4 *>(g.ws + w.partials);
+    int *mass_flag = reinterpret_cast<int *>(g.ws + Workspace::mass_flag);
+    g.generation = g.generation == 0x7fffffff ? 1 : g.generation + 1;
+    const int generation = g.generation;
+    stage_sources_kernel<<<(unsigned)((geo.n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, geo.n_pad, packed, mass_flag,
+                                                                              generation);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (geo.a_count == 0) {                      // more shares than blocks: this share delivers nothing
+        CUDA_TRY(cudaMemsetAsync(out, 0, (size_t)n * 16, st));
+        return COLATUS_OK;
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (g.profile) {
+        if (g.ev_used + 2 > g.ev_pool.size()) {
+            for (int i = 0; i < 64; ++i) {
+                cudaEvent_t e;
+                CUDA_TRY(cudaEventCreate(&e));
+                g.ev_pool.push_back(e);
+            }
+        }
+        e0 = g.ev_pool[g.ev_used++];
+        e1 = g.ev_pool[g.ev_used++];
+        CUDA_TRY(cudaEventRecord(e0, st));
+    }
+    for (int c = 0; c < geo.chunks; ++c) {
+        const int k_begin = 1 + c * geo.K;
+        const int k_count = geo.H - c * geo.K < geo.K ? geo.H - c * geo.K : geo.K;
+        CUDA_TRY(launch_force_sym(geo, packed, k_begin, k_count, c == 0, eps2, partials, mass_flag, generation, nullptr,
+                                  st, false));
+        g.launches++;
+        if (g.profile && c == 0 && geo.chunks == 1) CUDA_TRY(cudaEventRecord(e1, st));
+        if (c == 0)
+            reduce_sym_part_kernel<false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits, k_begin, k_count,
+                                                                  geo.nb, (int)geo.bt(), geo.a_begin, geo.a_count, 1, n,
+                                                                  (float)g.G, out);
+        else
+            reduce_sym_part_kernel<true><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits, k_begin, k_count,
+                                                                 geo.nb, (int)geo.bt(), geo.a_begin, geo.a_count, 0, n,
+                                                                 (float)g.G, out);
+        CUDA_TRY(cudaGetLastError());
+        g.launches++;
+    }
+    if (g.profile && geo.chunks > 1) CUDA_TRY(cudaEventRecord(e1, st));
+    return COLATUS_OK;
+}
+
 // The branch-free self term (reading G4) is exactly 0 only while w = m_k rinv^3 stays finite in FP32 (0 * inf = NaN):
 // rinv^3 = eps2^-1.5 <= 1e36 at this floor, which leaves masses up to ~3e2 in magnitude (colatus.h "eps2").
 inline bool eps2_ok(float eps2) { return std::isfinite(eps2) && eps2 >= 1e-24f; }
@@ -544,24 +609,29 @@ int enqueue_drift(double d) {
     return COLATUS_OK;
 }
 
-int enqueue_force_kick_drift(double cv, double ck, double d2, float tag) {
-    int rc = run_forces(g.pos, g.n, g.t_begin, g.t_count, g.eps2, g.acc, false, g.stream);
-    if (rc) return rc;
+// eqs. (4)-(5) for the target range from forces in `acc` (float4[t_count], indexed from the range's first body)
+int enqueue_kick_drift(const float4 *acc, double cv, double ck, double d2, float tag) {
     const unsigned blocks = (unsigned)((g.t_count + 255) / 256);
     if (g.trace_k > 0) {
         const Workspace w = workspace_layout(g.n);
         const int32_t *slot = reinterpret_cast<const int32_t *>(g.ws + w.trace_slot);
         float4 *row = g.ring + (size_t)(g.step % g.trace_cap) * g.trace_k;
-        kick_drift_kernel<true><<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, (float)cv,
+        kick_drift_kernel<true><<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, acc, g.t_begin, g.t_count, (float)cv,
                                                               (float)ck, (float)d2, slot, row, tag);
     } else {
-        kick_drift_kernel<false><<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, g.acc, g.t_begin, g.t_count, (float)cv,
+        kick_drift_kernel<false><<<blocks, 256, 0, g.stream>>>(g.pos, g.vel, acc, g.t_begin, g.t_count, (float)cv,
                                                                (float)ck, (float)d2, nullptr, nullptr, tag);
     }
     CUDA_TRY(cudaGetLastError());
     g.launches++;
     g.step++;
     return COLATUS_OK;
+}
+
+int enqueue_force_kick_drift(double cv, double ck, double d2, float tag) {
+    int rc = run_forces(g.pos, g.n, g.t_begin, g.t_count, g.eps2, g.acc, false, g.stream);
+    if (rc) return rc;
+    return enqueue_kick_drift(g.acc, cv, ck, d2, tag);
 }
 
 // Whole-range step without external terms: three launches (drift+stage, force, reduce+kick+drift).
@@ -806,6 +876,15 @@ int colatus_forces_range(const void *pos_mass_dev, int64_t n, int64_t target_beg
     if (rc) return rc;
     return run_forces(static_cast<const float4 *>(pos_mass_dev), n, target_begin, target_count, eps2,
                       static_cast<float4 *>(acc_out_dev), false, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int colatus_forces_symmetric_part(const void *pos_mass_dev, int64_t n, float eps2, int part, int parts,
+                                  void *acc_out_dev, void *cuda_stream) {
+    int rc = check_forces_args(pos_mass_dev, n, 0, n, eps2, acc_out_dev);
+    if (rc) return rc;
+    if (parts < 1 || part < 0 || part >= parts) return fail(COLATUS_INVALID_ARG, "need 0 <= part < parts");
+    return run_forces_sym_part(static_cast<const float4 *>(pos_mass_dev), n, eps2, part, parts,
+                               static_cast<float4 *>(acc_out_dev), static_cast<cudaStream_t>(cuda_stream));
 }
 
 int colatus_forces_host(const float *pos_mass_host, int64_t n, float eps2, float *acc_out_host, void *cuda_stream) {
@@ -1104,6 +1183,15 @@ int colatus_force_kick_drift(double cv, double ck, double d2) {
     if (!std::isfinite(cv) || !std::isfinite(ck) || !std::isfinite(d2))
         return fail(COLATUS_INVALID_ARG, "non-finite step coefficient");
     return enqueue_force_kick_drift(cv, ck, d2, 0.f);
+}
+
+int colatus_kick_drift(const void *acc_dev, double cv, double ck, double d2) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!acc_dev || !aligned16(acc_dev)) return fail(COLATUS_INVALID_ARG, "acc_dev null or misaligned");
+    if (!std::isfinite(cv) || !std::isfinite(ck) || !std::isfinite(d2))
+        return fail(COLATUS_INVALID_ARG, "non-finite step coefficient");
+    return enqueue_kick_drift(static_cast<const float4 *>(acc_dev), cv, ck, d2, 0.f);
 }
 
 int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_steps) {

@@ -153,18 +153,22 @@ __device__ __forceinline__ SymTile sym_tile_at(int p, int a, int nb, int k_begin
     return t;
 }
 
-// grid = (NB blocks, S splits).  staged = the source array padded to NB * BT bodies (far-away zero-mass padding);
+// grid = (blocks of this launch, S splits): target blocks a_begin .. a_begin + gridDim.x - 1 of the NB blocks (all of
+// them for a whole evaluation; a share of them when the evaluation is divided over GPUs or calls,
+// colatus_forces_symmetric_part).  staged = the source array padded to NB * BT bodies (far-away zero-mass padding);
 // targets are read from it too.  Split s works on positions [s * P / S, (s + 1) * P / S) of the block's list of
 // P = TPB * (k_count + (with_plain ? 1 + (NB even) : 0)) tiles.  Output rows of `stride` float4: row s =
 // target-side sums of split s (all NB * BT targets); row S + (k - k_begin) = reaction sums (already negated) of
-// block distance k.  Every row is written in full by every launch.
+// block distance k.  A launch over all NB blocks writes every row in full; a launch over a share of the blocks writes
+// the target-side rows of its own blocks and, in reaction row k, the blocks b = a + k (mod NB) of its blocks a --
+// reduce_sym_part_kernel adds exactly those cells.
 // BODY: 0 = both tile bodies in the kernel, picked by the equal-mass flag; 1 = general body only, 2 = equal-mass
 // body only -- such a kernel returns at once when the flag asks for the other body, so launching the pair (1, 2) is
 // the same evaluation with each body scheduled by ptxas on its own (the two bodies in one kernel cost each other
 // 1-2.5 %); worth the second, empty launch for large problems only.
 template <int IP, int TJ, int NST, int MINB, int BODY>
 __global__ void __launch_bounds__(FORCE_THREADS, MINB)
-force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_begin, int k_count, int with_plain,
+force_sym_kernel(const float4 *__restrict__ staged, int nb, int a_begin, int splits, int k_begin, int k_count, int with_plain,
                  float eps2, float4 *__restrict__ partial, int64_t stride, const int *__restrict__ mass_flag,
                  int generation, int *__restrict__ step_ctr) {
     constexpr int TILE_BYTES = TJ * 16;
@@ -179,7 +183,7 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
     float *racc_all = reinterpret_cast<float *>(acc2 + (size_t)IP * 3 * FORCE_THREADS);   // [NW][3][TJ]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int a = blockIdx.x, s = blockIdx.y;
+    const int a = a_begin + blockIdx.x, s = blockIdx.y;
     if (BODY != 0) {                 // uniform over the grid; before any barrier or copy is set up
         griddep_wait();
         if ((__ldg(mass_flag) != generation) != (BODY == 2)) return;
@@ -225,7 +229,7 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
     for (int c = 0; c < IP * 3; ++c) acc2[c * FORCE_THREADS + tid] = 0ull;
     float *racc = racc_all + (size_t)warp * 3 * TJ;
     for (int j = lane; j < 3 * TJ; j += 32) racc[j] = 0.f;
-    if (step_ctr && tid == FORCE_THREADS - 1 && a == 0 && s == 0) step_ctr[1] = step_ctr[0];
+    if (step_ctr && tid == FORCE_THREADS - 1 && blockIdx.x == 0 && s == 0) step_ctr[1] = step_ctr[0];
     const bool eqm = __ldg(mass_flag) != generation;
     const float m_common = eqm ? __ldg(staged).w : 1.0f;        // applied once to the finished sums
     __syncwarp();
@@ -306,6 +310,53 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
         o[t] = make_float4(fx[0] * m_common, fy[0] * m_common, fz[0] * m_common, 0.f);
         o[t + 1] = make_float4(fx[1] * m_common, fy[1] * m_common, fz[1] * m_common, 0.f);
     }
+}
+
+// Fixed-order sum of the cells a launch over target blocks [a_begin, a_begin + a_count) has written (above), for
+// every body t < n: the S target-side rows if t's block is one of the launch's, then reaction row k for every block
+// distance k of the launch whose source block b - k (mod NB) is one of the launch's.  FP64 accumulation, one rounding,
+// x G.  ACCUM adds to out (later chunks of block distances).  Summed over a partition of the blocks, the outputs are
+// the whole force: this is what a GPU contributes before the all-reduce of the sharded symmetric evaluation.
+template <bool ACCUM>
+__global__ void __launch_bounds__(256)
+reduce_sym_part_kernel(const float4 *__restrict__ partial, int64_t stride, int splits, int k_begin, int k_count, int nb,
+                       int block_bodies, int a_begin, int a_count, int with_plain, int64_t n, float G,
+                       float4 *__restrict__ out) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const int b = (int)(t / block_bodies);
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    int rel = b - a_begin;
+    if (rel < 0) rel += nb;
+    if (rel < a_count) {
+        (void)with_plain;               // the target-side rows hold 0 for a launch without one-directional tiles too
+        for (int s = 0; s < splits; ++s) {
+            const float4 q = partial[(size_t)s * stride + t];
+            sx += (double)q.x;
+            sy += (double)q.y;
+            sz += (double)q.z;
+        }
+    }
+    for (int dk = 0; dk < k_count; ++dk) {
+        int a = b - (k_begin + dk);
+        if (a < 0) a += nb;
+        int ra = a - a_begin;
+        if (ra < 0) ra += nb;
+        if (ra < a_count) {
+            const float4 q = partial[(size_t)(splits + dk) * stride + t];
+            sx += (double)q.x;
+            sy += (double)q.y;
+            sz += (double)q.z;
+        }
+    }
+    float4 r = make_float4((float)sx * G, (float)sy * G, (float)sz * G, 0.f);
+    if (ACCUM) {
+        const float4 o = out[t];
+        r.x += o.x;
+        r.y += o.y;
+        r.z += o.z;
+    }
+    out[t] = r;
 }
 
 }  // namespace colatus

@@ -97,3 +97,117 @@ def test_sharded_two_slices_evaluated_one_after_the_other_equal_the_full_step():
     assert np.abs(out_v[:, :3] - v_ref[:, :3]).max() <= 2e-5 * vr
     assert np.abs(out_x[:, :3] - x_ref[:, :3]).max() <= 1e-6
     assert not np.array_equal(out_x[:, :3], pm[:, :3])
+
+
+# ---- the symmetric evaluation divided over GPUs (colatus_forces_symmetric_part; sharded.py symmetric mode) ---------
+@pytest.mark.parametrize("block", [1024, 1536])
+@pytest.mark.parametrize("parts", [1, 2, 3, 5, 8])
+def test_symmetric_parts_add_up_to_the_whole_force(parts, block):
+    """Each share of the block pairs, evaluated on this GPU one after the other (what the ranks of a `parts`-GPU run
+    compute at the same time): the partial forces on ALL bodies add up to the oracle's forces; shares of different
+    sizes (blocks not divisible by parts), even and odd block counts, chunked block distances."""
+    import torch
+    from paper_1208_3444_b200.harness import Session
+    cfg, pm, _ = inputs.make_config(4, n_override=21000)            # log-normal masses, clusters
+    ref = oracle.forces(pm, cfg.eps2, 1.0)
+    rms = np.sqrt((ref ** 2).sum(1).mean())
+    with Session(1.0, cfg.n) as s:
+        B.colatus_set_option("symmetric_block", block)
+        pm_d = s.to_device(pm)
+        for rows in (0, 7):
+            B.colatus_set_option("symmetric_rows", rows)
+            total = np.zeros((cfg.n, 3))
+            reached = np.zeros(cfg.n, dtype=bool)
+            for part in range(parts):
+                out = torch.full((cfg.n, 4), np.nan, dtype=torch.float32, device=pm_d.device)
+                B.colatus_forces_symmetric_part(pm_d, cfg.n, cfg.eps2, part, parts, out)
+                o = out.cpu().numpy()
+                assert np.isfinite(o).all() and np.all(o[:, 3] == 0.0)
+                total += o[:, :3].astype(np.float64)
+                reached |= np.any(o[:, :3] != 0.0, axis=1)
+            assert reached.all()
+            d = np.linalg.norm(total - ref, axis=1)
+            assert np.median(d / np.linalg.norm(ref, axis=1)) <= 1e-5 and d.max() / rms <= 1e-4, (parts, block, rows)
+        with pytest.raises(B.ColatusError):
+            B.colatus_forces_symmetric_part(pm_d, cfg.n, cfg.eps2, parts, parts, out)
+
+
+def test_symmetric_shares_are_disjoint_in_what_they_own():
+    """With 14 shares of 14 blocks (H = 6) share 0 is block 0: it delivers to itself (its own sums, incl. the
+    one-directional term of the antipodal block 7 acting on IT) and reactions to the 6 blocks after it; every other
+    body gets exactly 0 from it (the all-reduce adds exact zeros there)."""
+    import torch
+    from paper_1208_3444_b200.harness import Session
+    cfg, pm, _ = inputs.make_config(3, n_override=14 * 1536)
+    with Session(1.0, cfg.n) as s:
+        B.colatus_set_option("symmetric_block", 1536)
+        pm_d = s.to_device(pm)
+        out = torch.empty((cfg.n, 4), dtype=torch.float32, device=pm_d.device)
+        B.colatus_forces_symmetric_part(pm_d, cfg.n, cfg.eps2, 0, 14, out)       # share 0 = block 0
+        o = out.cpu().numpy().reshape(14, 1536, 4)
+        nonzero = [bool(np.any(o[b, :, :3] != 0.0)) for b in range(14)]
+        assert nonzero == [True] * 7 + [False] * 7
+
+
+def test_sharded_stepper_symmetric_mode_world1_and_two_emulated_ranks():
+    """ShardedStepper in symmetric mode through the C ABI at world size 1 (10 steps of config 1 against the oracle,
+    tracer rows bit-exact), and one step of a 2-rank run emulated on this GPU: both ranks' shares of the pairs summed
+    (the all-reduce), then each rank's kick-drift of its own slice -- equal to the world-size-1 step to rounding."""
+    import torch
+    from paper_1208_3444_b200.harness import Session
+    from paper_1208_3444_b200.sharded import LibcolatusOps, ShardedStepper
+    cfg, pm, vel = inputs.make_config(1)
+    steps = 10
+    tr = np.arange(0, cfg.n, cfg.n // 16, dtype=np.int32)
+    mids, _ = oracle.midstep_schedule(cfg.cosmo, cfg.a_start, cfg.tau, steps)
+    with Session(cfg.G, cfg.n) as s:
+        pos, v = s.to_device(pm), s.to_device(vel)
+        ops = LibcolatusOps(pos, v, torch.zeros_like(pos), cfg.n, cfg.eps2, 0, cfg.n)
+        stepper = ShardedStepper(pos, cfg.n, ops, symmetric=True)
+        assert stepper.symmetric and stepper.acc_full.shape == pos.shape
+        idx = torch.from_numpy(tr).to(pos.device)
+        ring = torch.zeros((steps, tr.size, 4), dtype=torch.float32, device=pos.device)
+        ops.trace(idx, ring, steps)
+        for a, H in mids:
+            stepper.step(cfg.tau, a, H)
+        rows = stepper.trace_read(tr, 0, steps)
+        torch.cuda.synchronize()
+        x_gpu, v_gpu = pos.cpu().numpy(), v.cpu().numpy()
+        assert stepper.reduces == 0 and stepper.gathers == 0
+    st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+    for a, H in mids:
+        st.step(cfg.tau, a, H)
+    assert np.linalg.norm(x_gpu[:, :3].astype(np.float64) - st.x, axis=1).max() <= 1e-5          # G16
+    assert np.array_equal(rows[-1, :, :3], v_gpu[tr, :3])
+
+    c = B.colatus_step_coefficients(cfg.tau, 0.05, 3.0)
+    half = cfg.n // 2
+    rng = np.random.Generator(np.random.PCG64(5))
+    vel2 = vel.copy()
+    vel2[:, :3] = 0.05 * rng.standard_normal((cfg.n, 3)).astype(np.float32)
+    with Session(cfg.G, cfg.n) as s:
+        pos, v = s.to_device(pm), s.to_device(vel2)
+        one = ShardedStepper(pos, cfg.n, LibcolatusOps(pos, v, torch.zeros_like(pos), cfg.n, cfg.eps2, 0, cfg.n),
+                             symmetric=True)
+        one.step_coeffs(*c)
+        torch.cuda.synchronize()
+        x_ref, v_ref = pos.cpu().numpy(), v.cpu().numpy()
+        # two ranks: drift both slices, "all-gather", both shares of the pairs, "all-reduce", kick-drift per slice
+        pos, v = s.to_device(pm), s.to_device(vel2)
+        acc = torch.zeros((half, 4), dtype=torch.float32, device=pos.device)
+        B.colatus_upload(pos, v, acc, cfg.n, cfg.eps2)
+        for b in (0, half):
+            B.colatus_set_target_range(b, half)
+            B.colatus_drift(c[0])
+        parts = [torch.empty_like(pos) for _ in range(2)]
+        for r in range(2):
+            B.colatus_forces_symmetric_part(pos, cfg.n, cfg.eps2, r, 2, parts[r])
+        total = parts[0] + parts[1]
+        for b in (0, half):
+            B.colatus_set_target_range(b, half)
+            B.colatus_kick_drift(total[b:b + half], c[1], c[2], c[3])
+        torch.cuda.synchronize()
+        x2, v2 = pos.cpu().numpy(), v.cpu().numpy()
+    vr = float(np.sqrt((v_ref[:, :3].astype(np.float64) ** 2).sum(1).mean()))
+    assert np.abs(v2[:, :3] - v_ref[:, :3]).max() <= 2e-5 * vr and np.abs(x2[:, :3] - x_ref[:, :3]).max() <= 1e-6
+    assert not np.array_equal(x2[:, :3], pm[:, :3])

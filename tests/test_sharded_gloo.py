@@ -81,6 +81,52 @@ class OracleSliceOps:
     def trace_rows(self, first_step, n_steps):
         return self.ring[first_step:first_step + n_steps].copy()
 
+    # ---- symmetric mode: this rank's share of the unordered pairs, on ALL bodies; then the kick from given forces
+    BLOCK = 32                       # bodies per block of the stand-in's circulant pairing
+
+    def forces_symmetric_part(self, part, parts, acc_full):
+        """Same division of the work as colatus_forces_symmetric_part (target blocks [nb part / parts, nb (part+1) /
+        parts); block a meets a+1 .. a+H both ways, itself and -- nb even -- the antipodal block one way), in FP64
+        with numpy: the pair term is computed ONCE and added to both bodies."""
+        x, m = self.pos[:, :3].numpy(), self.pos[:, 3].numpy()
+        n, B_ = x.shape[0], self.BLOCK
+        nb = (n + B_ - 1) // B_
+        H = (nb - 1) // 2
+        F = np.zeros((n, 3))
+        blk = lambda b: np.arange(b * B_, min((b + 1) * B_, n))
+
+        def one_way(ti, sj):
+            d = x[sj][None, :, :] - x[ti][:, None, :]
+            s2 = (d * d).sum(2) + self.eps2
+            w = m[sj][None, :] / (s2 * np.sqrt(s2))
+            w[ti[:, None] == sj[None, :]] = 0.0
+            F[ti] += self.G * (w[:, :, None] * d).sum(1)
+
+        for a in range(nb * part // parts, nb * (part + 1) // parts):
+            ti = blk(a)
+            one_way(ti, ti)
+            if nb % 2 == 0 and nb > 1:
+                one_way(ti, blk((a + nb // 2) % nb))
+            for k in range(1, H + 1):
+                sj = blk((a + k) % nb)
+                d = x[sj][None, :, :] - x[ti][:, None, :]
+                s2 = (d * d).sum(2) + self.eps2
+                g = d / (s2 * np.sqrt(s2))[:, :, None]                     # the antisymmetric pair term, once
+                F[ti] += self.G * (m[sj][None, :, None] * g).sum(1)        # action
+                F[sj] -= self.G * (m[ti][:, None, None] * g).sum(0)        # reaction
+        acc_full[:, :3] = torch.from_numpy(F)
+        acc_full[:, 3] = 0.0
+
+    def kick_drift(self, acc_slice, cv, ck, d2):
+        self.vel.mul_(cv).add_(ck * acc_slice[:, :3])
+        s = slice(self.begin, self.begin + self.count)
+        self.pos[s, :3] += d2 * self.vel
+        for t, k in enumerate(TRACERS):
+            if self.begin <= k < self.begin + self.count:
+                self.ring[self.step, t, :3] = self.vel[k - self.begin].numpy()
+                self.ring[self.step, t, 3] = 1.0
+        self.step += 1
+
 
 def _free_port():
     with socket.socket() as s:
@@ -88,7 +134,7 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, pm, vel, eps2, G, coeffs, out_dir):
+def _worker(rank, world, port, pm, vel, eps2, G, coeffs, out_dir, symmetric=False):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -96,11 +142,13 @@ def _worker(rank, world, port, pm, vel, eps2, G, coeffs, out_dir):
         pos = torch.from_numpy(pm.astype(np.float64))
         begin, count = partition(pm.shape[0], world, rank)
         v = torch.from_numpy(vel[begin:begin + count, :3].astype(np.float64))
-        stepper = ShardedStepper(pos, pm.shape[0], OracleSliceOps(pos, v, eps2, G, begin, count, len(coeffs)))
-        assert (stepper.begin, stepper.count) == (begin, count)
+        stepper = ShardedStepper(pos, pm.shape[0], OracleSliceOps(pos, v, eps2, G, begin, count, len(coeffs)),
+                                 symmetric=symmetric)
+        assert (stepper.begin, stepper.count) == (begin, count) and stepper.symmetric == symmetric
         for c in coeffs:
             stepper.step_coeffs(*c)
         assert stepper.gathers == len(coeffs) and stepper.dirty          # ONE all-gather per step
+        assert stepper.reduces == (len(coeffs) if symmetric else 0)       # symmetric mode: + ONE all-reduce of forces
         other = slice(0, count) if rank == 1 else slice(count, 2 * count)
         stale = pos[other].clone()
         d_kin = stepper.diagnostics(0.5)                                  # no potential: no gather needed
@@ -124,7 +172,10 @@ def test_partition():
         partition(1000, 3, 0)
 
 
-def test_two_rank_sharded_stepping_matches_single_process(tmp_path):
+@pytest.mark.parametrize("symmetric", [False, True])
+def test_two_rank_sharded_stepping_matches_single_process(tmp_path, symmetric):
+    """symmetric=False: eq. (1) divided by targets; True: by block pairs, every pair evaluated once by one of the two
+    ranks, action and reaction delivered by one all-reduce of the partial forces (sharded.py)."""
     cfg, pm, vel = inputs.make_config(1, n_override=N)
     rng = np.random.Generator(np.random.PCG64(7))
     vel = vel.copy()
@@ -135,7 +186,7 @@ def test_two_rank_sharded_stepping_matches_single_process(tmp_path):
         coeffs.append((0.5 * cfg.tau, (1 - H * cfg.tau) / (1 + H * cfg.tau),
                        cfg.tau / (a ** 3 * (1 + H * cfg.tau)), 0.5 * cfg.tau))
 
-    mp.spawn(_worker, args=(WORLD, _free_port(), pm, vel, float(cfg.eps2), cfg.G, coeffs, str(tmp_path)),
+    mp.spawn(_worker, args=(WORLD, _free_port(), pm, vel, float(cfg.eps2), cfg.G, coeffs, str(tmp_path), symmetric),
              nprocs=WORLD, join=True)
 
     ref = oracle.State(pm, vel, cfg.eps2, cfg.G)
@@ -147,9 +198,10 @@ def test_two_rank_sharded_stepping_matches_single_process(tmp_path):
     pos0 = np.load(tmp_path / "pos0.npy")
     pos1 = np.load(tmp_path / "pos1.npy")
     assert np.array_equal(pos0, pos1)                      # every rank ends with the same full position array
-    assert np.abs(pos0[:, :3] - ref.x).max() <= 1e-14      # same arithmetic, per-target sums in the same order
+    # target sharding: same arithmetic, per-target sums in the same order; pair sharding: another summation order (FP64)
+    assert np.abs(pos0[:, :3] - ref.x).max() <= (1e-12 if symmetric else 1e-14)
     v = np.concatenate([np.load(tmp_path / "vel0.npy"), np.load(tmp_path / "vel1.npy")])
-    assert np.abs(v - ref.v).max() <= 1e-13
+    assert np.abs(v - ref.v).max() <= (1e-10 if symmetric else 1e-13)
     assert np.array_equal(pos0[:, 3], pm[:, 3].astype(np.float64))   # masses untouched by the exchange
 
     # diagnostics: one all-reduce of the 16 doubles gives the whole-system sums on every rank
