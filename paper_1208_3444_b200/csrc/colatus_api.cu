@@ -310,11 +310,11 @@ Geometry choose_geometry(int64_t n, int64_t t_count, bool potential = false) {
 // device), or -- from SYM_PAIR_N bodies on -- two launches, a general-only and an equal-mass-only kernel, of which the
 // one the equal-mass flag does not ask for returns at once (15 us at 2^20): compiled alone the general body runs
 // 2.4 % faster (94.0 % against 91.8 % of peak at 2^20; the equal-mass body is the same either way).
-template <int IP, int TJ, int BODY>
-cudaError_t launch_force_sym_body(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
+template <int IP, int TJ, int BODY, bool PART>
+cudaError_t launch_force_sym_inst(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
                                   float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
                                   cudaStream_t st, bool pdl) {
-    auto kern = force_sym_kernel<IP, TJ, NSTAGES, 2, BODY>;
+    auto kern = force_sym_kernel<IP, TJ, NSTAGES, 2, BODY, PART>;
     const size_t smem = force_sym_smem_bytes<IP, TJ, NSTAGES>();
     static int attr_epoch = 0;
     if (attr_epoch != g.init_epoch) {
@@ -323,8 +323,20 @@ cudaError_t launch_force_sym_body(const Geometry &geo, const float4 *packed, int
         attr_epoch = g.init_epoch;
     }
     dim3 grid((unsigned)geo.a_count, (unsigned)geo.splits);
-    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, packed, geo.nb, geo.a_begin, geo.splits, k_begin,
-                     k_count, with_plain, eps2, partials, geo.n_pad, mass_flag, generation, step_ctr);
+    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, pdl, packed, geo.nb, geo.splits, k_begin, k_count,
+                     with_plain, eps2, partials, geo.n_pad, mass_flag, generation, step_ctr, geo.a_begin);
+}
+
+// whole evaluations (all nb target blocks) and shares of one (colatus_forces_symmetric_part) are separate instantiations
+template <int IP, int TJ, int BODY>
+cudaError_t launch_force_sym_body(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
+                                  float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
+                                  cudaStream_t st, bool pdl) {
+    if (geo.a_begin == 0 && geo.a_count == geo.nb)
+        return launch_force_sym_inst<IP, TJ, BODY, false>(geo, packed, k_begin, k_count, with_plain, eps2, partials,
+                                                          mass_flag, generation, step_ctr, st, pdl);
+    return launch_force_sym_inst<IP, TJ, BODY, true>(geo, packed, k_begin, k_count, with_plain, eps2, partials,
+                                                     mass_flag, generation, step_ctr, st, pdl);
 }
 
 inline bool sym_pair(const Geometry &geo) { return geo.n_pad >= SYM_PAIR_N; }
@@ -381,6 +393,24 @@ cudaError_t launch_force(const Geometry &geo, const float4 *pos_mass, const floa
     }
 }
 
+// colatus_profile: take an event pair from the pool, record the first on `st` now; the caller records *end after the
+// last force-kernel launch of the evaluation (left null when profiling is off).
+int profile_begin(cudaStream_t st, cudaEvent_t *end) {
+    *end = nullptr;
+    if (!g.profile) return COLATUS_OK;
+    if (g.ev_used + 2 > g.ev_pool.size()) {
+        for (int i = 0; i < 64; ++i) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreate(&e));
+            g.ev_pool.push_back(e);
+        }
+    }
+    cudaEvent_t begin = g.ev_pool[g.ev_used++];
+    *end = g.ev_pool[g.ev_used++];
+    CUDA_TRY(cudaEventRecord(begin, st));
+    return COLATUS_OK;
+}
+
 // stage + force (+ reduce): the whole of step a3.  No validation here.
 // `fused` (whole-range steps only): the staging pass also applies the drift of eq. (3) to the resident
 // positions (drift_stage_kernel), and the partial-sum reduction is left to the caller's fused
@@ -433,19 +463,8 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         g.launches++;
     }
 
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (g.profile) {
-        if (g.ev_used + 2 > g.ev_pool.size()) {
-            for (int i = 0; i < 64; ++i) {
-                cudaEvent_t e;
-                CUDA_TRY(cudaEventCreate(&e));
-                g.ev_pool.push_back(e);
-            }
-        }
-        e0 = g.ev_pool[g.ev_used++];
-        e1 = g.ev_pool[g.ev_used++];
-        CUDA_TRY(cudaEventRecord(e0, st));
-    }
+    cudaEvent_t e1 = nullptr;                   // colatus_profile: bracket this evaluation's force-kernel launches
+    if (int rc = profile_begin(st, &e1)) return rc;
     int *step_ctr = fused ? fused->step_ctr : nullptr;
     if (geo.sym) {
         // every pair once (force_sym_kernels.cuh): one launch per chunk of block distances; its rows (target-side
@@ -548,19 +567,8 @@ int run_forces_sym_part(const float4 *pos_mass, int64_t n, float eps2, int part,
         CUDA_TRY(cudaMemsetAsync(out, 0, (size_t)n * 16, st));
         return COLATUS_OK;
     }
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (g.profile) {
-        if (g.ev_used + 2 > g.ev_pool.size()) {
-            for (int i = 0; i < 64; ++i) {
-                cudaEvent_t e;
-                CUDA_TRY(cudaEventCreate(&e));
-                g.ev_pool.push_back(e);
-            }
-        }
-        e0 = g.ev_pool[g.ev_used++];
-        e1 = g.ev_pool[g.ev_used++];
-        CUDA_TRY(cudaEventRecord(e0, st));
-    }
+    cudaEvent_t e1 = nullptr;                   // colatus_profile: bracket this evaluation's force-kernel launches
+    if (int rc = profile_begin(st, &e1)) return rc;
     for (int c = 0; c < geo.chunks; ++c) {
         const int k_begin = 1 + c * geo.K;
         const int k_count = geo.H - c * geo.K < geo.K ? geo.H - c * geo.K : geo.K;

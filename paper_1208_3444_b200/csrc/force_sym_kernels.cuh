@@ -76,7 +76,7 @@ __device__ __forceinline__ void sym_tile_body(const unsigned char *tile, const u
                 const u64 r3 = mul2(rinv, rinv2);
                 const u64 wi = EQM ? r3 : mul2(r3, M);
                 const u64 wj = EQM ? r3 : mul2(r3, mi[i]);
-ax[i] = fma2(wi, dx, ax[i]);
+                ax[i] = fma2(wi, dx, ax[i]);
                 ay[i] = fma2(wi, dy, ay[i]);
                 az[i] = fma2(wi, dz, az[i]);
                 rx = fma2(wj, dx, rx);
@@ -166,11 +166,14 @@ __device__ __forceinline__ SymTile sym_tile_at(int p, int a, int nb, int k_begin
 // body only -- such a kernel returns at once when the flag asks for the other body, so launching the pair (1, 2) is
 // the same evaluation with each body scheduled by ptxas on its own (the two bodies in one kernel cost each other
 // 1-2.5 %); worth the second, empty launch for large problems only.
-template <int IP, int TJ, int NST, int MINB, int BODY>
+// PART: the launch covers the target blocks a_begin .. a_begin + gridDim.x - 1 only (a share of the evaluation).  A
+// template parameter, and a_begin the LAST argument, because the mere use of a_begin in the whole-evaluation kernel
+// moved ptxas's schedule of the tile loop: 319.3 ms against 313.7 ms at N = 2^20 (profiles/r02_symmetric_kernel.md).
+template <int IP, int TJ, int NST, int MINB, int BODY, bool PART>
 __global__ void __launch_bounds__(FORCE_THREADS, MINB)
-force_sym_kernel(const float4 *__restrict__ staged, int nb, int a_begin, int splits, int k_begin, int k_count, int with_plain,
+force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_begin, int k_count, int with_plain,
                  float eps2, float4 *__restrict__ partial, int64_t stride, const int *__restrict__ mass_flag,
-                 int generation, int *__restrict__ step_ctr) {
+                 int generation, int *__restrict__ step_ctr, int a_begin) {
     constexpr int TILE_BYTES = TJ * 16;
     constexpr int BT = FORCE_THREADS * 2 * IP;
     constexpr int TPB = BT / TJ;
@@ -183,7 +186,7 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int a_begin, int spl
     float *racc_all = reinterpret_cast<float *>(acc2 + (size_t)IP * 3 * FORCE_THREADS);   // [NW][3][TJ]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int a = a_begin + blockIdx.x, s = blockIdx.y;
+    const int a = PART ? a_begin + (int)blockIdx.x : (int)blockIdx.x, s = blockIdx.y;
     if (BODY != 0) {                 // uniform over the grid; before any barrier or copy is set up
         griddep_wait();
         if ((__ldg(mass_flag) != generation) != (BODY == 2)) return;
