@@ -241,3 +241,36 @@ def test_plan_of_the_baseline_configurations(session):
         assert big["partial_rows"] * big["padded_bodies"] * 16 <= 8 << 30
         assert B.colatus_force_plan(1 << 20, 1 << 19)["symmetric"] == 0          # target sub-range
         assert B.colatus_force_plan(1 << 20, None, True)["symmetric"] == 0       # potential
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_symmetric_kernel_fuzz_against_the_one_directional_kernel(session, symmetric_always, seed):
+    """Seeded random problem sizes (2 .. 70000: 1 to 69 blocks, odd and even), block sizes, split counts and row caps
+    (1 to ~20 launches), equal and general masses, scales and offsets: the symmetric evaluation agrees with the
+    one-directional kernel -- which test_gpu_forces.py holds to the oracle at every size -- far inside the bars, and
+    with the oracle itself where it is cheap (n <= 20000)."""
+    rng = np.random.Generator(np.random.PCG64(4400 + seed))
+    n = int(rng.integers(2, 70000)) if seed % 4 else int(rng.integers(2, 5000))
+    block = (0, 1024, 1536)[int(rng.integers(0, 3))]
+    splits = int(rng.integers(0, 17))
+    scale = 10.0 ** rng.uniform(-2, 2)
+    pm = _problem(n, bool(seed % 2), seed=seed)
+    pm[:, :3] = (scale * (pm[:, :3] + rng.uniform(-20, 20, size=3))).astype(np.float32)
+    eps2 = np.float32((scale * 10.0 ** rng.uniform(-3, -1.5)) ** 2)
+    B.colatus_set_option("symmetric_block", block)
+    B.colatus_set_option("source_splits", splits)
+    plan = B.colatus_force_plan(n)
+    if plan["distances"] > 2 and seed % 3 == 0:
+        B.colatus_set_option("symmetric_rows", plan["splits"] + int(rng.integers(1, plan["distances"])))
+        plan = B.colatus_force_plan(n)
+    assert plan["symmetric"] == 1
+    sym = session.forces(pm, eps2).cpu().numpy()
+    B.colatus_set_option("symmetric", 0)
+    B.colatus_set_option("source_splits", 0)
+    plain = session.forces(pm, eps2).cpu().numpy()
+    ref = plain[:, :3].astype(np.float64)
+    med, mx = force_errors(sym[:, :3], ref)
+    assert med <= 2e-6 and mx <= 2e-5, (seed, n, block, splits, plan, med, mx)
+    if n <= 20000:
+        med, mx = force_errors(sym[:, :3], oracle.forces(pm, eps2, 1.0))
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL, (seed, n, med, mx)
