@@ -73,6 +73,8 @@ def parse():
                     help="4 = N=2^20 (the reported workload, default); 5 = N=2^22 (the at-scale case of BASELINE.json); "
                          "2, 3 = the equal-mass stepping configurations (N = 32768, 131072), for profiling the equal-mass loop")
     ap.add_argument("--n", type=int, default=0, help="override N (debug only; the reported workload is 2^20)")
+    ap.add_argument("--sharded-driver", action="store_true",
+                    help="run the multi-GPU step driver (sharded.py) even at N = 1: a self-test of that code path on one GPU")
     return ap.parse_args()
 
 
@@ -253,7 +255,7 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
     sess.upload(pm, vel, cfg.eps2)
     tr_idx = (np.arange(N_TRACERS, dtype=np.int64) * (n // N_TRACERS)).astype(np.int32)
     stepper = None
-    if world > 1:
+    if world > 1 or args.sharded_driver:
         sess.acc = torch.zeros((count, 4), dtype=torch.float32, device=sess.device)
         ops = LibcolatusOps(sess.pos, sess.vel, sess.acc, n, cfg.eps2, begin, count)
         stepper = ShardedStepper(sess.pos, n, ops)
