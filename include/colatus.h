@@ -311,16 +311,16 @@ int64_t  colatus_launch_count(void);
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 
 /* Which force kernel an evaluation of target_count targets out of n bodies takes (eq. 1).
- * Whole-range evaluations (target_count == n) without the potential and with at least 24576 bodies use the
- * SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
+ * Whole-range evaluations (target_count == n) of at least 24576 bodies use the SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
  * per unordered pair and applied to both bodies (Newton's third law) -- 16 packed FP32 operations per
  * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 1536 (1024 below 65536 bodies); block a meets the `distances`
  * blocks a+1 .. a+distances (mod blocks) both ways, and itself (and the antipodal block when `blocks` is even)
  * one way.  The sums a block receives from each distance are kept as partial rows in the workspace and
  * added in fixed row order (in FP64 when there are more than 16 rows), so results are reproducible bit for
  * bit; when the rows of all distances exceed 8 GiB the evaluation runs as `launches` kernel launches of
- * `distances_per_launch` distances each.  Target sub-ranges, potential evaluations and smaller problems take
- * the one-directional kernel (out[0] = 0; its geometry is colatus_force_geometry's).
+ * `distances_per_launch` distances each.  Potential evaluations (with_potential != 0) carry the potential as a
+ * fourth component through the same kernel, always with 1024-body blocks.  Target sub-ranges and smaller
+ * problems take the one-directional kernel (out[0] = 0; its geometry is colatus_force_geometry's).
  * out[0] = 1 symmetric / 0 one-directional, out[1] = blocks, out[2] = splits of a block's work (CTAs = blocks x
  * splits), out[3] = distances H = (blocks-1)/2, out[4] = distances per launch, out[5] = launches,
  * out[6] = padded bodies, out[7] = partial rows added per body (0: none). */

@@ -250,14 +250,15 @@ Geometry choose_plain_geometry(int64_t n, int64_t t_count) {
 // of cost model as above in units of one symmetric tile: (tiles per CTA) * (CTAs per SM + ramp) + CTAs per SM * c0.
 // K = block distances per launch = what the partial rows of workspace_layout(n) hold; a pure function of n.
 bool sym_eligible(int64_t n, int64_t t_count, bool potential) {
-    if (g.symmetric == 0 || potential || t_count != n || g.force_I != 0) return false;
+    (void)potential;            // potential evaluations take the symmetric kernel too (its 1024-body variant)
+    if (g.symmetric == 0 || t_count != n || g.force_I != 0) return false;
     return g.symmetric == 2 || n >= SYM_MIN_N;
 }
 
-Geometry choose_sym_geometry(int64_t n, int part = 0, int parts = 1) {
+Geometry choose_sym_geometry(int64_t n, int part = 0, int parts = 1, bool potential = false) {
     Geometry geo;
     geo.sym = true;
-    geo.IP = sym_ip(n);
+    geo.IP = potential ? 2 : sym_ip(n);      // the potential's fourth component fits the 128 registers with 4 targets/thread
     geo.TJ = geo.IP == 3 ? 512 : 256;
     geo.nb = (int)sym_blocks(n, geo.IP);
     geo.a_begin = (int)((int64_t)geo.nb * part / parts);
@@ -300,7 +301,7 @@ Geometry choose_sym_geometry(int64_t n, int part = 0, int parts = 1) {
 
 Geometry choose_geometry(int64_t n, int64_t t_count, bool potential = false) {
     if (sym_eligible(n, t_count, potential)) {
-        const Geometry geo = choose_sym_geometry(n);
+        const Geometry geo = choose_sym_geometry(n, 0, 1, potential);
         if (geo.sym) return geo;
     }
     return choose_plain_geometry(n, t_count);
@@ -356,6 +357,22 @@ cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_be
     g.launches++;
     return launch_force_sym_body<3, 512, 2>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
                                             generation, step_ctr, st, pdl);
+}
+
+// potential evaluations: the 1024-body variant with the fourth (potential) component, both tile bodies in one kernel
+cudaError_t launch_force_sym_pot(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
+                                 float eps2, float4 *partials, const int *mass_flag, int generation, cudaStream_t st) {
+    auto kern = force_sym_pot_kernel<2, 256, NSTAGES, 2>;
+    const size_t smem = force_sym_pot_smem_bytes<2, 256, NSTAGES>();
+    static int attr_epoch = 0;
+    if (attr_epoch != g.init_epoch) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_epoch = g.init_epoch;
+    }
+    dim3 grid((unsigned)geo.a_count, (unsigned)geo.splits);
+    return launch_ex(kern, grid, dim3(FORCE_THREADS), smem, st, false, packed, geo.nb, geo.splits, k_begin, k_count,
+                     with_plain, eps2, partials, geo.n_pad, mass_flag, generation);
 }
 
 template <int IP, int TJ, bool POT>
@@ -475,8 +492,12 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
         for (int c = 0; c < geo.chunks; ++c) {
             const int k_begin = 1 + c * geo.K;
             const int k_count = geo.H - c * geo.K < geo.K ? geo.H - c * geo.K : geo.K;
-            CUDA_TRY(launch_force_sym(geo, packed, k_begin, k_count, c == 0, eps2, partials, mass_flag, generation,
-                                      c == 0 ? step_ctr : nullptr, st, fused && fused->pdl && c == 0));
+            if (potential)
+                CUDA_TRY(launch_force_sym_pot(geo, packed, k_begin, k_count, c == 0, eps2, partials, mass_flag,
+                                              generation, st));
+            else
+                CUDA_TRY(launch_force_sym(geo, packed, k_begin, k_count, c == 0, eps2, partials, mass_flag, generation,
+                                          c == 0 ? step_ctr : nullptr, st, fused && fused->pdl && c == 0));
             g.launches++;
             if (fused && geo.chunks == 1) {
                 if (g.profile) CUDA_TRY(cudaEventRecord(e1, st));
@@ -485,7 +506,13 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
                 return COLATUS_OK;
             }
             if (c == 0 && g.profile && geo.chunks == 1) CUDA_TRY(cudaEventRecord(e1, st));
-            if (c == 0)
+            if (potential && c == 0)      // the j = k term of the diagonal tiles is removed once, with the first chunk
+                reduce_partials_kernel<true, false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
+                                                                            (float)g.G, eps2, pos_mass, 0, out);
+            else if (potential)
+                reduce_sym_pot_more_kernel<<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
+                                                                   (float)g.G, out);
+            else if (c == 0)
                 reduce_partials_kernel<false, false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
                                                                              (float)g.G, eps2, pos_mass, 0, out);
             else

@@ -315,6 +315,294 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
     }
 }
 
+// ---- the same evaluation with the potential (colatus_forces_potential, the W of colatus_diagnostics) -----------------
+template <int IP, int TJ, int NST>
+constexpr size_t force_sym_pot_smem_bytes() {
+    return (size_t)NST * TJ * 16 + 2 * NST * sizeof(uint64_t) + (size_t)IP * 4 * FORCE_THREADS * 8 +
+           (size_t)4 * (FORCE_THREADS / 32) * TJ * 4;
+}
+
+// sym_tile_body with the potential as a fourth component: racc = this warp's reaction sums [4][TJ] (x, y, z, pot).
+// A function of its own (and a kernel of its own below) rather than a template flag of sym_tile_body: any edit of
+// that function's text, even one compiled out, moves ptxas's schedule of the force-only loop (profiles/r02_symmetric_kernel.md 3b).  mi = the masses of the thread's own target pairs (general
+// loop only).  POT: also sum_j m_j / sqrt(r^2 + eps^2) on the target side and sum_k m_k / sqrt(...) on the source side
+// (the potential is symmetric in the pair, not antisymmetric: no sign change for the reaction).
+template <int IP, int TJ, bool EQM>
+__device__ __forceinline__ void sym_tile_body_pot(const unsigned char *tile, const u64 (&nx)[IP], const u64 (&ny)[IP],
+                                              const u64 (&nz)[IP], const u64 (&mi)[IP], u64 eps2_2, u64 (&ax)[IP],
+                                              u64 (&ay)[IP], u64 (&az)[IP], u64 (&ap)[IP], float *racc, int lane) {
+    const int f = (lane >> 2) & 7;
+    // Position p reads source p ^ f of the 128-byte row of 8 sources.  Two ways to form the address, measured on the
+    // B200 (N = 2^20, % of peak by the 20-flop convention): eight per-lane byte offsets (p ^ f) * 16 kept in registers
+    // (equal-mass body: 104.4 against 102.8), or the lane's row pointer plus a per-bit signed offset -- p ^ f =
+    // f + sum over the set bits b of p of (f has b ? -b : +b) -- which needs no extra registers (general body:
+    // 94.2 against 91.5); the first formulation, ((jb + p) ^ f) << 4 computed per load, gave 92.9 / 101.4.
+    constexpr bool POT = true;
+    int q[8];
+    if (EQM) {
+#pragma unroll
+        for (int p = 0; p < 8; ++p) q[p] = (p << 4) ^ (f << 4);
+    }
+    for (int jb = 0; jb < TJ; jb += 8) {
+        float vx[8], vy[8], vz[8], vp[POT ? 8 : 1];
+        const unsigned char *row = tile + (jb << 4) + (f << 4);   // this lane's source at position 0
+#pragma unroll
+        for (int p = 0; p < 8; ++p) {
+            const int off = ((p & 1) ? ((f & 1) ? -16 : 16) : 0) + ((p & 2) ? ((f & 2) ? -32 : 32) : 0) +
+                            ((p & 4) ? ((f & 4) ? -64 : 64) : 0);
+            const float4 S = EQM ? *reinterpret_cast<const float4 *>(tile + (jb << 4) + q[p])
+                                 : *reinterpret_cast<const float4 *>(row + off);
+            const u64 X = pack2(S.x, S.x), Y = pack2(S.y, S.y), Z = pack2(S.z, S.z), M = pack2(S.w, S.w);
+            u64 rx = 0ull, ry = 0ull, rz = 0ull, rp = 0ull;
+#pragma unroll
+            for (int i = 0; i < IP; ++i) {
+                const u64 dx = add2(nx[i], X);
+                const u64 dy = add2(ny[i], Y);
+                const u64 dz = add2(nz[i], Z);
+                u64 r2 = fma2(dz, dz, eps2_2);
+                r2 = fma2(dy, dy, r2);
+                r2 = fma2(dx, dx, r2);
+                float r2a, r2b;
+                unpack2(r2, r2a, r2b);
+                const u64 rinv = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));
+                const u64 rinv2 = mul2(rinv, rinv);
+                const u64 r3 = mul2(rinv, rinv2);
+                const u64 wi = EQM ? r3 : mul2(r3, M);
+                const u64 wj = EQM ? r3 : mul2(r3, mi[i]);
+                ax[i] = fma2(wi, dx, ax[i]);
+                ay[i] = fma2(wi, dy, ay[i]);
+                az[i] = fma2(wi, dz, az[i]);
+                rx = fma2(wj, dx, rx);
+                ry = fma2(wj, dy, ry);
+                rz = fma2(wj, dz, rz);
+                if (POT) {
+                    ap[i] = add2(ap[i], EQM ? rinv : mul2(rinv, M));
+                    rp = EQM ? add2(rp, rinv) : fma2(rinv, mi[i], rp);
+                }
+            }
+            float lo, hi;
+            unpack2(rx, lo, hi);
+            vx[p] = lo + hi;
+            unpack2(ry, lo, hi);
+            vy[p] = lo + hi;
+            unpack2(rz, lo, hi);
+            vz[p] = lo + hi;
+            if (POT) {
+                unpack2(rp, lo, hi);
+                vp[p] = lo + hi;
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            vx[p] += __shfl_xor_sync(0xffffffffu, vx[p + 4], 16);
+            vy[p] += __shfl_xor_sync(0xffffffffu, vy[p + 4], 16);
+            vz[p] += __shfl_xor_sync(0xffffffffu, vz[p + 4], 16);
+            if (POT) vp[p] += __shfl_xor_sync(0xffffffffu, vp[POT ? p + 4 : 0], 16);
+        }
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            vx[p] += __shfl_xor_sync(0xffffffffu, vx[p + 2], 8);
+            vy[p] += __shfl_xor_sync(0xffffffffu, vy[p + 2], 8);
+            vz[p] += __shfl_xor_sync(0xffffffffu, vz[p + 2], 8);
+            if (POT) vp[p] += __shfl_xor_sync(0xffffffffu, vp[POT ? p + 2 : 0], 8);
+        }
+        vx[0] += __shfl_xor_sync(0xffffffffu, vx[1], 4);
+        vy[0] += __shfl_xor_sync(0xffffffffu, vy[1], 4);
+        vz[0] += __shfl_xor_sync(0xffffffffu, vz[1], 4);
+        vx[0] += __shfl_xor_sync(0xffffffffu, vx[0], 2);
+        vy[0] += __shfl_xor_sync(0xffffffffu, vy[0], 2);
+        vz[0] += __shfl_xor_sync(0xffffffffu, vz[0], 2);
+        vx[0] += __shfl_xor_sync(0xffffffffu, vx[0], 1);
+        vy[0] += __shfl_xor_sync(0xffffffffu, vy[0], 1);
+        vz[0] += __shfl_xor_sync(0xffffffffu, vz[0], 1);
+        if (POT) {
+            vp[0] += __shfl_xor_sync(0xffffffffu, vp[POT ? 1 : 0], 4);
+            vp[0] += __shfl_xor_sync(0xffffffffu, vp[0], 2);
+            vp[0] += __shfl_xor_sync(0xffffffffu, vp[0], 1);
+        }
+        if ((lane & 3) == 0) {                           // lane l now holds the warp's sum for source jb + f(l)
+            racc[jb + f] += vx[0];
+            racc[TJ + jb + f] += vy[0];
+            racc[2 * TJ + jb + f] += vz[0];
+            if (POT) racc[3 * TJ + jb + f] += vp[0];
+        }
+    }
+}
+
+// POT: rows carry the potential sums in .w (target side: sum_j m_j / sqrt(r^2 + eps^2) including the j = k term of the
+// diagonal tiles, which the row reduction removes; reaction rows: the same sum over the block's partners).
+template <int IP, int TJ, int NST, int MINB>
+__global__ void __launch_bounds__(FORCE_THREADS, MINB)
+force_sym_pot_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_begin, int k_count, int with_plain,
+                 float eps2, float4 *__restrict__ partial, int64_t stride, const int *__restrict__ mass_flag,
+                 int generation) {
+    constexpr bool POT = true, PART = false;
+    constexpr int BODY = 0;
+    int *const step_ctr = nullptr;
+    const int a_begin = 0;
+    constexpr int TILE_BYTES = TJ * 16;
+    constexpr int BT = FORCE_THREADS * 2 * IP;
+    constexpr int TPB = BT / TJ;
+    constexpr int NW = FORCE_THREADS / 32;
+    static_assert(BT % TJ == 0, "a block is a whole number of tiles");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem_raw + NST * TILE_BYTES);
+    uint64_t *empty_bar = full_bar + NST;
+    constexpr int NC = POT ? 4 : 3;                                                   // components per body
+    u64 *acc2 = reinterpret_cast<u64 *>(smem_raw + NST * TILE_BYTES + 2 * NST * 8);   // [IP*NC][THREADS]
+    float *racc_all = reinterpret_cast<float *>(acc2 + (size_t)IP * NC * FORCE_THREADS);   // [NW][NC][TJ]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int a = PART ? a_begin + (int)blockIdx.x : (int)blockIdx.x, s = blockIdx.y;
+    if (BODY != 0) {                 // uniform over the grid; before any barrier or copy is set up
+        griddep_wait();
+        if ((__ldg(mass_flag) != generation) != (BODY == 2)) return;
+    }
+    const int P = TPB * (k_count + (with_plain ? ((nb & 1) ? 1 : 2) : 0));
+    const int p0 = (int)(((int64_t)s * P) / splits), p1 = (int)(((int64_t)(s + 1) * P) / splits);
+    const unsigned char *src = reinterpret_cast<const unsigned char *>(staged);
+
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NST; ++q) {
+            mbar_init(&full_bar[q], 1);
+            mbar_init(&empty_bar[q], NW);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    griddep_wait();
+    griddep_launch_dependents();
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < NST; ++q)
+            if (p0 + q < p1) {
+                const SymTile t = sym_tile_at<TPB>(p0 + q, a, nb, k_begin, k_count, with_plain);
+                mbar_arrive_expect_tx(&full_bar[q], TILE_BYTES);
+                bulk_copy_g2s(smem_raw + q * TILE_BYTES, src + (size_t)t.tile * TILE_BYTES, TILE_BYTES, &full_bar[q]);
+            }
+    }
+
+    u64 nx[IP], ny[IP], nz[IP], mi[IP];
+    const int64_t tbase = (int64_t)a * BT + 2 * tid;
+#pragma unroll
+    for (int i = 0; i < IP; ++i) {
+        const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
+        const float4 b0 = __ldg(staged + t), b1 = __ldg(staged + t + 1);
+        nx[i] = pack2(-b0.x, -b1.x);
+        ny[i] = pack2(-b0.y, -b1.y);
+        nz[i] = pack2(-b0.z, -b1.z);
+        mi[i] = pack2(b0.w, b1.w);
+    }
+    const u64 eps2_2 = pack2(eps2, eps2);
+#pragma unroll
+    for (int c = 0; c < IP * NC; ++c) acc2[c * FORCE_THREADS + tid] = 0ull;
+    float *racc = racc_all + (size_t)warp * NC * TJ;
+    for (int j = lane; j < NC * TJ; j += 32) racc[j] = 0.f;
+    if (step_ctr && tid == FORCE_THREADS - 1 && blockIdx.x == 0 && s == 0) step_ctr[1] = step_ctr[0];
+    const bool eqm = __ldg(mass_flag) != generation;
+    const float m_common = eqm ? __ldg(staged).w : 1.0f;        // applied once to the finished sums
+    __syncwarp();
+
+    for (int p = p0; p < p1; ++p) {
+        const int it = p - p0;
+        const int stage = it % NST;
+        const uint32_t parity = (it / NST) & 1;
+        const SymTile T = sym_tile_at<TPB>(p, a, nb, k_begin, k_count, with_plain);
+        mbar_wait(&full_bar[stage], parity);
+        const unsigned char *tile = smem_raw + (size_t)stage * TILE_BYTES;
+        u64 ax[IP], ay[IP], az[IP], ap[IP];
+#pragma unroll
+        for (int i = 0; i < IP; ++i) ax[i] = ay[i] = az[i] = ap[i] = 0ull;
+        if (T.k == 0) {
+            const float4 *tp = reinterpret_cast<const float4 *>(tile);
+            if (BODY == 2 || (BODY == 0 && eqm))
+                force_tile_body<IP, TJ, POT, true>(tp, nx, ny, nz, eps2_2, ax, ay, az, ap);
+            else
+                force_tile_body<IP, TJ, POT, false>(tp, nx, ny, nz, eps2_2, ax, ay, az, ap);
+        } else {
+            if (BODY == 2 || (BODY == 0 && eqm))
+                sym_tile_body_pot<IP, TJ, true>(tile, nx, ny, nz, mi, eps2_2, ax, ay, az, ap, racc, lane);
+            else
+                sym_tile_body_pot<IP, TJ, false>(tile, nx, ny, nz, mi, eps2_2, ax, ay, az, ap, racc, lane);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[stage]);
+        if (tid == 0 && p + NST < p1) {
+            const SymTile N = sym_tile_at<TPB>(p + NST, a, nb, k_begin, k_count, with_plain);
+            mbar_wait(&empty_bar[stage], parity);
+            mbar_arrive_expect_tx(&full_bar[stage], TILE_BYTES);
+            bulk_copy_g2s(smem_raw + stage * TILE_BYTES, src + (size_t)N.tile * TILE_BYTES, TILE_BYTES,
+                          &full_bar[stage]);
+        }
+#pragma unroll
+        for (int i = 0; i < IP; ++i) {
+            u64 *a2 = acc2 + (size_t)(i * NC) * FORCE_THREADS + tid;
+            a2[0] = add2(a2[0], ax[i]);
+            a2[FORCE_THREADS] = add2(a2[FORCE_THREADS], ay[i]);
+            a2[2 * FORCE_THREADS] = add2(a2[2 * FORCE_THREADS], az[i]);
+            if (POT) a2[3 * FORCE_THREADS] = add2(a2[3 * FORCE_THREADS], ap[i]);
+        }
+        if (T.k != 0) {
+            // reaction of this tile: add the 8 warps' sums in warp order, negate, write the row of distance k
+            __syncthreads();
+            int bb = a + T.k;
+            if (bb >= nb) bb -= nb;
+            float4 *row = partial + (size_t)(splits + T.k - k_begin) * stride + (size_t)bb * BT + (size_t)T.sub * TJ;
+            for (int j = tid; j < TJ; j += FORCE_THREADS) {
+                float sx = racc_all[j], sy = racc_all[TJ + j], sz = racc_all[2 * TJ + j];
+                float sp = POT ? racc_all[3 * TJ + j] : 0.f;
+#pragma unroll
+                for (int w = 1; w < NW; ++w) {
+                    sx += racc_all[(size_t)w * NC * TJ + j];
+                    sy += racc_all[(size_t)w * NC * TJ + TJ + j];
+                    sz += racc_all[(size_t)w * NC * TJ + 2 * TJ + j];
+                    if (POT) sp += racc_all[(size_t)w * NC * TJ + 3 * TJ + j];
+                }
+                row[j] = make_float4(-sx * m_common, -sy * m_common, -sz * m_common, sp * m_common);
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    racc_all[(size_t)w * NC * TJ + j] = 0.f;
+                    racc_all[(size_t)w * NC * TJ + TJ + j] = 0.f;
+                    racc_all[(size_t)w * NC * TJ + 2 * TJ + j] = 0.f;
+                    if (POT) racc_all[(size_t)w * NC * TJ + 3 * TJ + j] = 0.f;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    float4 *o = partial + (size_t)s * stride;
+#pragma unroll
+    for (int i = 0; i < IP; ++i) {
+        const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
+        const u64 *a2 = acc2 + (size_t)(i * NC) * FORCE_THREADS + tid;
+        float fx[2], fy[2], fz[2], fp[2] = {0.f, 0.f};
+        unpack2(a2[0], fx[0], fx[1]);
+        unpack2(a2[FORCE_THREADS], fy[0], fy[1]);
+        unpack2(a2[2 * FORCE_THREADS], fz[0], fz[1]);
+        if (POT) unpack2(a2[3 * FORCE_THREADS], fp[0], fp[1]);
+        o[t] = make_float4(fx[0] * m_common, fy[0] * m_common, fz[0] * m_common, fp[0] * m_common);
+        o[t + 1] = make_float4(fx[1] * m_common, fy[1] * m_common, fz[1] * m_common, fp[1] * m_common);
+    }
+}
+
+// Later chunks of a chunked POTENTIAL evaluation: out += G * (row sums), with out.w -= G * (potential row sums) -- the
+// first chunk went through reduce_partials_kernel<true>, which also removed the j = k term.
+__global__ void __launch_bounds__(256)
+reduce_sym_pot_more_kernel(const float4 *__restrict__ partial, int64_t stride, int rows, int64_t n, float G,
+                           float4 *__restrict__ out) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const float4 s = sum_partials(partial, stride, rows, t);
+    float4 o = out[t];
+    o.x += s.x * G;
+    o.y += s.y * G;
+    o.z += s.z * G;
+    o.w -= s.w * G;
+    out[t] = o;
+}
+
 // Fixed-order sum of the cells a launch over target blocks [a_begin, a_begin + a_count) has written (above), for
 // every body t < n: the S target-side rows if t's block is one of the launch's, then reaction row k for every block
 // distance k of the launch whose source block b - k (mod NB) is one of the launch's.  FP64 accumulation, one rounding,

@@ -240,7 +240,8 @@ def test_plan_of_the_baseline_configurations(session):
         assert big["symmetric"] == 1 and big["launches"] > 1
         assert big["partial_rows"] * big["padded_bodies"] * 16 <= 8 << 30
         assert B.colatus_force_plan(1 << 20, 1 << 19)["symmetric"] == 0          # target sub-range
-        assert B.colatus_force_plan(1 << 20, None, True)["symmetric"] == 0       # potential
+        pot = B.colatus_force_plan(1 << 20, None, True)                          # potential: 1024-body blocks, chunked
+        assert pot["symmetric"] == 1 and pot["blocks"] == 1024 and pot["launches"] == 2
 
 
 @pytest.mark.parametrize("seed", range(16))
@@ -276,30 +277,26 @@ def test_symmetric_kernel_fuzz_against_the_one_directional_kernel(session, symme
         assert med <= MEDIAN_TOL and mx <= MAX_TOL, (seed, n, med, mx)
 
 
-@pytest.mark.parametrize("index", [4, 5])
-def test_full_size_both_kernels_agree_on_every_target(index):
-    """BASELINE configs 4 (N = 2^20, the launch configuration bench.py times: 683 x 13 CTAs, one launch) and 5
-    (N = 2^22: 12 launches of 116 block distances): the oracle can check 4096 sampled targets (test_gpu_forces.py);
-    here EVERY target is compared between the symmetric and the one-directional kernel -- two independent
-    decompositions of eq. (1) -- so that no block, tile, split or chunk boundary of the full-size geometry can hide
-    between the samples."""
-    import torch
-    from paper_1208_3444_b200.harness import Session
-    cfg, pm, _ = inputs.make_config(index)
-    with Session(1.0, cfg.n) as s:
-        d = s.to_device(pm)
-        plan = B.colatus_force_plan(cfg.n)
-        assert plan["symmetric"] == 1 and plan["launches"] == (1 if index == 4 else 12)
-        sym = s.forces(d, cfg.eps2)
-        B.colatus_set_option("symmetric", 0)
-        plain = s.forces(d, cfg.eps2)
-        B.colatus_set_option("symmetric", 1)
-        diff = (sym[:, :3].double() - plain[:, :3].double()).norm(dim=1)
-        nr = plain[:, :3].double().norm(dim=1)
-        med = float((diff / nr).median())
-        mx = float(diff.max() / (nr ** 2).mean().sqrt())
-        worst_rel = float((diff / nr).max())
-        torch.cuda.synchronize()
-    record_parity(f"config {index}: symmetric vs one-directional kernel, all targets", n=cfg.n, targets=cfg.n,
-                  median_rel=med, max_over_rms=mx, worst_rel=worst_rel)
-    assert med <= 2e-6 and mx <= 2e-5, (med, mx)
+@pytest.mark.parametrize("equal_mass", [False, True])
+@pytest.mark.parametrize("n", [1, 2, 1025, 3073, 30000])
+def test_symmetric_kernel_with_the_potential(session, symmetric_always, n, equal_mass):
+    """colatus_forces_potential through the symmetric kernel (fourth component: the potential is symmetric in the
+    pair, the j = k term of the diagonal tiles is removed by the row reduction): forces and phi against the oracle,
+    one launch and chunked over block distances."""
+    pm = _problem(n, equal_mass, seed=100 + n)
+    eps2 = np.float32(1e-4)
+    plan = B.colatus_force_plan(n, None, True)
+    assert plan["symmetric"] == 1 and plan["blocks"] == (n + 1023) // 1024
+    ref, phi = oracle.forces(pm, eps2, 1.0, potential=True)
+    for rows in ((0, 5) if n == 30000 else (0,)):
+        B.colatus_set_option("symmetric_rows", rows)
+        if rows:
+            B.colatus_set_option("source_splits", 2)
+            assert B.colatus_force_plan(n, None, True)["launches"] == 5          # H = 14, 3 distances per launch
+        out = session.forces(pm, eps2, potential=True).cpu().numpy()
+        if n == 1:       # phi = -(m / eps - m / eps): the removed j = k term leaves at most its own rounding
+            assert np.all(out[:, :3] == 0.0) and abs(out[0, 3]) <= 2e-7 * pm[0, 3] / np.sqrt(eps2)
+            continue
+        med, mx = force_errors(out[:, :3], ref)
+        assert med <= MEDIAN_TOL and mx <= MAX_TOL, (n, equal_mass, rows, med, mx)
+        assert np.allclose(out[:, 3], phi, rtol=5e-5, atol=0), (n, equal_mass, rows)
