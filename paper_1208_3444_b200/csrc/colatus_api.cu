@@ -52,7 +52,7 @@ struct Geometry {
     int64_t tiles_t = 0;
     int splits = 0, tiles_per_split = 0;
     int64_t n_pad = 0;   // sources covered = splits * tiles_per_split * TJ
-    // symmetric kernel: nb blocks of SYM_BT bodies (n_pad = nb * SYM_BT, tiles_t = nb), H block distances,
+    // symmetric kernel: nb blocks of bt() bodies (n_pad = nb * bt(), tiles_t = nb), H block distances,
     // K of them per launch (K reaction rows + `splits` target-side rows in the workspace), `chunks` launches
     bool sym = false;
     int nb = 0, H = 0, K = 0, chunks = 0;

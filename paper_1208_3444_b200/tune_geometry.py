@@ -1,5 +1,6 @@
 #!/usr/bin/env python
-"""Launch-geometry sweep behind `choose_geometry` (csrc/colatus_api.cu; DESIGN.md 6.3 "Launch geometry").
+"""Launch-geometry sweep behind `choose_plain_geometry`, the one-directional force kernel's geometry
+(csrc/colatus_api.cu; DESIGN.md 6.3 "Launch geometry"; the symmetric kernel is switched off for the sweep).
 
     python -m paper_1208_3444_b200.tune_geometry [--sizes 4096,8192,...] [--fit] > profiles/rNN_geometry_sweep.md
 
@@ -32,6 +33,7 @@ def sweep(sizes, reps_us=20000.0):
     for n in sizes:
         cfg, pm, _ = inputs.make_config(1 if n < 262144 else 4, n)
         with Session(1.0, n) as s:
+            B.colatus_set_option("symmetric", 0)      # this tool sweeps the ONE-DIRECTIONAL kernel's geometry
             dev = s.to_device(pm)
             out = torch.empty_like(dev)
 
