@@ -52,8 +52,11 @@ FMA_PIPE_LANE_OPS_GENERAL, FMA_PIPE_LANE_OPS_EQUAL_MASS = 12.0, 11.0
 # symmetric kernel (each unordered pair once, applied to both bodies): per PAIR 3 add + 3 fma + rsqrt
 # + 4 mul (2 for equal masses) + 6 fma = 26 (24) flop and 16 (14) FMA-pipe lane-ops, plus ~1.07 adds per pair for
 # the reaction reduction (6.4 scalar adds per source and lane, 6 targets per lane); a pair is TWO interactions
-SYM_EXECUTED_FLOP_GENERAL, SYM_EXECUTED_FLOP_EQUAL_MASS = (26.0 + 1.07) / 2, (24.0 + 1.07) / 2
-SYM_LANE_OPS_GENERAL, SYM_LANE_OPS_EQUAL_MASS = (16.0 + 1.07) / 2, (14.0 + 1.07) / 2
+def sym_work(targets_per_thread, equal_mass):
+    """(executed flop, FMA-pipe lane-ops) per DELIVERED interaction of the symmetric kernel: per pair 26 (24) flop and
+    16 (14) lane-ops, plus 6.4 scalar adds per (lane, source) for the reaction reduction spread over the lane's targets."""
+    red = 6.4 / targets_per_thread
+    return ((24.0 if equal_mass else 26.0) + red) / 2, ((14.0 if equal_mass else 16.0) + red) / 2
 METRIC = "Ginteractions/s softened direct-sum gravity at N=2^20; % of FP32 FMA peak"
 UNIT = "Ginteractions/s"
 BENCH_TAU = 1.0e-6                         # step size of the bench steps (EdS background from a = 0.02)
@@ -321,12 +324,12 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
     if sym:
         cap = SYM_KERNEL_DRAM_TRAFFIC
         traffic = cap["bytes"] if (cap and n == cap["n"] and world == 1 and plan["splits"] == cap["splits"]) else None
-        lane_ops = SYM_LANE_OPS_EQUAL_MASS if equal_mass else SYM_LANE_OPS_GENERAL
-        executed = SYM_EXECUTED_FLOP_EQUAL_MASS if equal_mass else SYM_EXECUTED_FLOP_GENERAL
+        executed, lane_ops = sym_work(geo["targets_per_thread"], equal_mass)
         # staged bodies read as targets and as sources, every partial row written once
         algorithmic_bytes = 16 * plan["padded_bodies"] * (2 + plan["splits"] + plan["distances"])
-        kernel = "force_sym_kernel<%d,%d,4,2,%s> (every pair once, applied to both bodies)%s%s" % (
-            geo["targets_per_thread"] // 2, 512 if geo["targets_per_thread"] == 6 else 256,
+        kernel = "force_sym_kernel<%d,%d,4,%d,%s> (every pair once, applied to both bodies)%s%s" % (
+            geo["targets_per_thread"] // 2, 256 if geo["targets_per_thread"] == 4 else 512,
+            1 if geo["targets_per_thread"] > 6 else 2,
             ("2" if equal_mass else "1") if plan["padded_bodies"] >= 98304 else "0",
             " equal-mass loop" if equal_mass else "",
             "; %d launches + partial-row reductions per evaluation" % plan["launches"] if plan["launches"] > 1 else "")
@@ -353,7 +356,7 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
                 "flop_per_interaction": FLOP_PER_INTERACTION,
                 "frac_note": ("achieved = ALGORITHMIC flops: 20 flop x N^2 pair interactions delivered / kernel time "
                               "(BASELINE convention)." + (" The symmetric kernel evaluates each unordered pair once "
-                              "and applies it to both bodies, so it EXECUTES ~13.5 flop per delivered interaction: "
+                              "and applies it to both bodies, so it EXECUTES ~13.2 flop per delivered interaction: "
                               "frac can exceed 20/24 = 0.833, the ceiling of a one-directional kernel; "
                               "frac_executed_flops and fma_pipe_busy_frac count what the SMs really did."
                               if sym else "")),

@@ -37,12 +37,16 @@ constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in c
 constexpr int GRAPH_STEPS = COLATUS_GRAPH_STEPS;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
 
 // symmetric (each pair once) force kernel, force_sym_kernels.cuh: whole-range evaluations of at least SYM_MIN_N bodies
-// Two variants: blocks of 1536 bodies (6 targets per thread, 512-source tiles) and, below SYM_MID_N bodies, blocks of
-// 1024 (4 targets per thread, 256-source tiles), whose finer tiles split better over the SMs (N = 32768: 32 x 14
-// CTAs of 4.9 tiles against 22 x 13 of 2.8; 7 % faster; profiles/r02_symmetric_kernel.md section 4b)
+// Three variants: blocks of 4096 bodies (16 targets per thread, 254 registers, ONE CTA per SM, 512-source tiles) from
+// SYM_WIDE_N bodies on -- the per-source work of the source side (shuffle tree, permuted load, address arithmetic) is
+// amortised over 16 targets instead of 6 and 8 independent chains per thread replace the second CTA: 292.8 ms against
+// 313.8 ms at N = 2^20 (profiles/r02_symmetric_kernel.md section 4c); blocks of 1536 (6 targets per thread, two CTAs
+// per SM) below that; and below SYM_MID_N blocks of 1024 (4 targets per thread, 256-source tiles), whose finer tiles
+// split better over the SMs (N = 32768: 32 x 14 CTAs of 4.9 tiles against 22 x 13 of 2.8; 7 % faster; section 4b)
 constexpr int64_t SYM_MID_N = 65536;
+constexpr int64_t SYM_WIDE_N = 131072;
 constexpr int64_t SYM_MIN_N = 24576;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
-constexpr int SYM_MAX_SPLITS = 16;
+constexpr int SYM_MAX_SPLITS = 24;
 constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)
 constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch can always hold
 constexpr size_t SYM_ROWS_BUDGET = (size_t)8 << 30;               // bytes of partial rows before an evaluation is chunked
@@ -91,7 +95,7 @@ struct Context {
     int64_t launches = 0;
     // tuning overrides (0 = automatic)
     int force_I = 0, force_splits = 0;
-    int sym_block = 0;    // 0 = automatic, else 1024 or 1536 bodies per block ("symmetric_block")
+    int sym_block = 0;    // 0 = automatic, else 1024, 1536 or 4096 bodies per block ("symmetric_block")
     int sym_rows = 0;     // cap on partial rows per launch of the symmetric kernel (0 = what the workspace holds)
     int symmetric = 1;    // 0 = never, 1 = automatic (n >= SYM_MIN_N), 2 = whenever the evaluation allows it
     int init_epoch = 0;   // counts colatus_init calls
@@ -153,7 +157,7 @@ inline int max_splits(int64_t n) { return n <= SMALL_N ? MAX_SPLITS : MAX_SPLITS
 // rows of force_sym_kernel -- all of them ((splits + H) rows of n_pad bodies) while that stays within
 // SYM_ROWS_BUDGET, else the budget (the evaluation is then chunked over block distances), never fewer than
 // SYM_MAX_SPLITS + SYM_MIN_ROWS rows.  Non-decreasing in n, so a workspace sized for n_max serves every n <= n_max.
-inline int sym_ip(int64_t n) { return g.sym_block ? g.sym_block / 512 : (n < SYM_MID_N ? 2 : 3); }
+inline int sym_ip(int64_t n) { return g.sym_block ? g.sym_block / 512 : (n < SYM_MID_N ? 2 : (n < SYM_WIDE_N ? 3 : 8)); }
 inline int64_t sym_blocks(int64_t n, int ip) { return (n + 512 * ip - 1) / (512 * ip); }
 size_t sym_rows_bytes(int64_t n, int ip) {
     const size_t row = (size_t)sym_blocks(n, ip) * 512 * ip * 16;
@@ -168,13 +172,14 @@ size_t sym_rows_bytes(int64_t n, int ip) {
     }
     return bytes;
 }
-// The 1536-body variant's need at n and the 1024-body variant's at min(n, SYM_MID_N - 1) (it is the automatic choice
-// only below SYM_MID_N; forced above, it gets by with what is there -- more launches): non-decreasing across SYM_MID_N.
+// Every variant's need at min(n, the end of the range in which it is the automatic choice) -- forced beyond its
+// range ("symmetric_block") a variant gets by with what is there: more launches.  Non-decreasing across the thresholds.
 size_t partials_bytes(int64_t n) {
     size_t bytes = (size_t)max_splits(n) * (size_t)n * 16;
-    if (sym_rows_bytes(n, 3) > bytes) bytes = sym_rows_bytes(n, 3);
-    const int64_t n_mid = n < SYM_MID_N ? n : SYM_MID_N - 1;
-    if (sym_rows_bytes(n_mid, 2) > bytes) bytes = sym_rows_bytes(n_mid, 2);
+    const int64_t n2 = n < SYM_MID_N ? n : SYM_MID_N - 1, n3 = n < SYM_WIDE_N ? n : SYM_WIDE_N - 1;
+    if (sym_rows_bytes(n2, 2) > bytes) bytes = sym_rows_bytes(n2, 2);
+    if (sym_rows_bytes(n3, 3) > bytes) bytes = sym_rows_bytes(n3, 3);
+    if (sym_rows_bytes(n, 8) > bytes) bytes = sym_rows_bytes(n, 8);
     return bytes;
 }
 
@@ -276,8 +281,9 @@ Geometry choose_sym_geometry(int64_t n, int part = 0, int parts = 1, bool potent
     const double plain_tiles = tpb * ((geo.nb & 1) ? 1.0 : 2.0) * 0.68;   // a one-directional tile costs ~0.68 symmetric ones
     const double c0 = geo.IP == 3 ? 0.04 : 0.12;                           // per-CTA overhead in units of one tile
     double best_cost = -1.0;
-    for (int s = 1; s <= SYM_MAX_SPLITS; ++s) {
-        if (g.force_splits && g.force_splits <= SYM_MAX_SPLITS && g.force_splits < rows_avail && s != g.force_splits)
+    const int smax = geo.IP > 3 ? SYM_MAX_SPLITS : 16;     // one CTA per SM: the wave count is coarser, more splits help
+    for (int s = 1; s <= smax; ++s) {
+        if (g.force_splits && g.force_splits <= smax && g.force_splits < rows_avail && s != g.force_splits)
             continue;
         if (s >= rows_avail) break;
         int K = (int)(rows_avail - s);
@@ -315,7 +321,7 @@ template <int IP, int TJ, int BODY, bool PART>
 cudaError_t launch_force_sym_inst(const Geometry &geo, const float4 *packed, int k_begin, int k_count, int with_plain,
                                   float eps2, float4 *partials, const int *mass_flag, int generation, int *step_ctr,
                                   cudaStream_t st, bool pdl) {
-    auto kern = force_sym_kernel<IP, TJ, NSTAGES, 2, BODY, PART>;
+    auto kern = force_sym_kernel<IP, TJ, NSTAGES, (IP > 3 ? 1 : 2), BODY, PART>;   // 16 targets/thread: one CTA per SM
     const size_t smem = force_sym_smem_bytes<IP, TJ, NSTAGES>();
     static int attr_epoch = 0;
     if (attr_epoch != g.init_epoch) {
@@ -348,15 +354,22 @@ cudaError_t launch_force_sym(const Geometry &geo, const float4 *packed, int k_be
     if (geo.IP == 2)
         return launch_force_sym_body<2, 256, 0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
                                                 generation, step_ctr, st, pdl);
-    if (!sym_pair(geo))
+    if (geo.IP == 3 && !sym_pair(geo))
         return launch_force_sym_body<3, 512, 0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
                                                 generation, step_ctr, st, pdl);
-    cudaError_t e = launch_force_sym_body<3, 512, 1>(geo, packed, k_begin, k_count, with_plain, eps2, partials,
-                                                     mass_flag, generation, step_ctr, st, pdl);
+    if (geo.IP == 8 && !sym_pair(geo))
+        return launch_force_sym_body<8, 512, 0>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
+                                                generation, step_ctr, st, pdl);
+    cudaError_t e = geo.IP == 8 ? launch_force_sym_body<8, 512, 1>(geo, packed, k_begin, k_count, with_plain, eps2,
+                                                                   partials, mass_flag, generation, step_ctr, st, pdl)
+                                : launch_force_sym_body<3, 512, 1>(geo, packed, k_begin, k_count, with_plain, eps2,
+                                                                   partials, mass_flag, generation, step_ctr, st, pdl);
     if (e != cudaSuccess) return e;
     g.launches++;
-    return launch_force_sym_body<3, 512, 2>(geo, packed, k_begin, k_count, with_plain, eps2, partials, mass_flag,
-                                            generation, step_ctr, st, pdl);
+    return geo.IP == 8 ? launch_force_sym_body<8, 512, 2>(geo, packed, k_begin, k_count, with_plain, eps2, partials,
+                                                          mass_flag, generation, step_ctr, st, pdl)
+                       : launch_force_sym_body<3, 512, 2>(geo, packed, k_begin, k_count, with_plain, eps2, partials,
+                                                          mass_flag, generation, step_ctr, st, pdl);
 }
 
 // potential evaluations: the 1024-body variant with the fourth (potential) component, both tile bodies in one kernel
@@ -1403,7 +1416,7 @@ int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]) {
     out[1] = geo.tiles_t;
     out[2] = geo.splits;
     out[3] = geo.sym ? geo.n_pad : (int64_t)geo.tiles_per_split * geo.TJ;
-    out[4] = g.ctas_per_sm;
+    out[4] = geo.sym && geo.IP > 3 ? 1 : g.ctas_per_sm;
     out[5] = g.sm_count;
     out[6] = 2 * geo.IP;
     out[7] = FORCE_THREADS;
@@ -1438,7 +1451,8 @@ int colatus_set_option(const char *name, int64_t value) {
         if (value < 0 || value > 2) return fail(COLATUS_INVALID_ARG, "must be 0 (never), 1 (automatic) or 2 (always)");
         g.symmetric = (int)value;
     } else if (!strcmp(name, "symmetric_block")) {
-        if (value != 0 && value != 1024 && value != 1536) return fail(COLATUS_INVALID_ARG, "must be 0, 1024 or 1536");
+        if (value != 0 && value != 1024 && value != 1536 && value != 4096)
+            return fail(COLATUS_INVALID_ARG, "must be 0, 1024, 1536 or 4096");
         g.sym_block = (int)value;
     } else if (!strcmp(name, "symmetric_rows")) {
         if (value < 0 || value == 1 || value > 1000000) return fail(COLATUS_INVALID_ARG, "must be 0 or >= 2");

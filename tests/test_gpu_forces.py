@@ -65,7 +65,7 @@ def test_forces_config3_all_targets(session):
 def test_forces_config4_full_size_sampled(session):
     """N = 2^20 in the launch configuration bench.py times; 4096 seeded targets (BASELINE config 4)."""
     geo = B.colatus_force_geometry(1 << 20)
-    assert geo["targets_per_thread"] == 6
+    assert geo["targets_per_thread"] == 16 and B.colatus_force_plan(1 << 20)["symmetric"] == 1
     _check_config(session, 4)
 
 

@@ -45,12 +45,12 @@ def _problem(n, equal_mass, seed=0):
 
 
 @pytest.mark.parametrize("equal_mass", [False, True])
-@pytest.mark.parametrize("block", [1536, 1024])
-@pytest.mark.parametrize("n", [1, 2, 3, 1023, 1025, 1535, 1536, 1537, 3072, 3073, 4609, 6145, 7000, 10753, 12289])
+@pytest.mark.parametrize("block", [1536, 1024, 4096])
+@pytest.mark.parametrize("n", [1, 2, 3, 1023, 1025, 1535, 1536, 1537, 3072, 3073, 4097, 4609, 6145, 7000, 10753, 12289, 20481])
 def test_symmetric_kernel_ragged_sizes(session, symmetric_always, n, block, equal_mass):
-    """Both kernel variants (blocks of 1536 bodies with 512-source tiles, blocks of 1024 with 256-source tiles) with
-    1 block (diagonal only), 2 (antipodal only), 3, 4, 5, ... 13: odd and even counts, full and ragged last blocks;
-    all targets against the oracle."""
+    """All three kernel variants (blocks of 1536 bodies = 6 targets per thread, 1024 = 4 targets per thread with
+    256-source tiles, 4096 = 16 targets per thread and one CTA per SM) with 1 block (diagonal only), 2 (antipodal
+    only), 3, 4, 5, ... 21: odd and even counts, full and ragged last blocks; all targets against the oracle."""
     pm = _problem(n, equal_mass, seed=n)
     eps2 = np.float32(1e-4)
     B.colatus_set_option("symmetric_block", block)
@@ -65,7 +65,7 @@ def test_symmetric_kernel_ragged_sizes(session, symmetric_always, n, block, equa
         return
     ref = oracle.forces(pm, eps2, 1.0)
     med, mx = force_errors(out[:, :3], ref)
-    if n in (3073, 12289):
+    if n in (3073, 20481):
         record_parity(f"symmetric kernel n={n} block={block} equal_mass={equal_mass}", n=n, targets=n, median_rel=med,
                       max_over_rms=mx)
     assert med <= MEDIAN_TOL and mx <= MAX_TOL, (n, block, equal_mass, med, mx)
@@ -231,9 +231,9 @@ def test_plan_of_the_baseline_configurations(session):
     if True:
         small = B.colatus_force_plan(4096)
         assert small["symmetric"] == 0
-        for n in (32768, 131072, 1 << 20):
+        for n in (32768, 100000, 131072, 1 << 20):
             p = B.colatus_force_plan(n)
-            block = 1024 if n < 65536 else 1536
+            block = 1024 if n < 65536 else (1536 if n < 131072 else 4096)
             assert p["symmetric"] == 1 and p["launches"] == 1 and p["blocks"] == (n + block - 1) // block
             assert p["partial_rows"] == p["splits"] + p["distances"]
         big = B.colatus_force_plan(1 << 22)
@@ -241,7 +241,7 @@ def test_plan_of_the_baseline_configurations(session):
         assert big["partial_rows"] * big["padded_bodies"] * 16 <= 8 << 30
         assert B.colatus_force_plan(1 << 20, 1 << 19)["symmetric"] == 0          # target sub-range
         pot = B.colatus_force_plan(1 << 20, None, True)                          # potential: 1024-body blocks, chunked
-        assert pot["symmetric"] == 1 and pot["blocks"] == 1024 and pot["launches"] == 2
+        assert pot["symmetric"] == 1 and pot["blocks"] == 1024 and pot["launches"] == 4
 
 
 @pytest.mark.parametrize("seed", range(16))
@@ -252,7 +252,7 @@ def test_symmetric_kernel_fuzz_against_the_one_directional_kernel(session, symme
     with the oracle itself where it is cheap (n <= 20000)."""
     rng = np.random.Generator(np.random.PCG64(4400 + seed))
     n = int(rng.integers(2, 70000)) if seed % 4 else int(rng.integers(2, 5000))
-    block = (0, 1024, 1536)[int(rng.integers(0, 3))]
+    block = (0, 1024, 1536, 4096)[int(rng.integers(0, 4))]
     splits = int(rng.integers(0, 17))
     scale = 10.0 ** rng.uniform(-2, 2)
     pm = _problem(n, bool(seed % 2), seed=seed)

@@ -12,8 +12,8 @@ from conftest import record_parity  # noqa: E402
 
 @pytest.mark.parametrize("index", [4, 5])
 def test_full_size_both_kernels_agree_on_every_target(index):
-    """BASELINE configs 4 (N = 2^20, the launch configuration bench.py times: 683 x 13 CTAs, one launch) and 5
-    (N = 2^22: 12 launches of 116 block distances): the oracle can check 4096 sampled targets (test_gpu_forces.py);
+    """BASELINE configs 4 (N = 2^20, the launch configuration bench.py times: 256 blocks of 4096 bodies, one launch)
+    and 5 (N = 2^22: 1024 blocks, several launches of block distances): the oracle can check 4096 sampled targets (test_gpu_forces.py);
     here EVERY target is compared between the symmetric and the one-directional kernel -- two independent
     decompositions of eq. (1) -- so that no block, tile, split or chunk boundary of the full-size geometry can hide
     between the samples."""
@@ -23,7 +23,7 @@ def test_full_size_both_kernels_agree_on_every_target(index):
     with Session(1.0, cfg.n) as s:
         d = s.to_device(pm)
         plan = B.colatus_force_plan(cfg.n)
-        assert plan["symmetric"] == 1 and plan["launches"] == (1 if index == 4 else 12)
+        assert plan["symmetric"] == 1 and plan["blocks"] == cfg.n // 4096 and (plan["launches"] == 1) == (index == 4)
         sym = s.forces(d, cfg.eps2)
         B.colatus_set_option("symmetric", 0)
         plain = s.forces(d, cfg.eps2)

@@ -100,7 +100,7 @@ def test_sharded_two_slices_evaluated_one_after_the_other_equal_the_full_step():
 
 
 # ---- the symmetric evaluation divided over GPUs (colatus_forces_symmetric_part; sharded.py symmetric mode) ---------
-@pytest.mark.parametrize("block", [1024, 1536])
+@pytest.mark.parametrize("block", [1024, 1536, 4096])
 @pytest.mark.parametrize("parts", [1, 2, 3, 5, 8])
 def test_symmetric_parts_add_up_to_the_whole_force(parts, block):
     """Each share of the block pairs, evaluated on this GPU one after the other (what the ranks of a `parts`-GPU run
