@@ -43,7 +43,7 @@ FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.
 # summarised in profiles/: valid only for the (n, source splits) it was captured at -- reported as null otherwise.
 FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8, "symmetric": 0,
                              "profile": "profiles/r02_force_kernel_ncu_full.txt"}
-SYM_KERNEL_DRAM_TRAFFIC = {"bytes": 361063936 + 5896358000, "n": 1 << 20, "splits": 13,
+SYM_KERNEL_DRAM_TRAFFIC = {"bytes": 254605824 + 2335484000, "n": 1 << 20, "splits": 15,
                            "profile": "profiles/r02_force_sym_kernel_ncu_full.txt"}
 # executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
 # (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention

@@ -86,7 +86,7 @@ typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosm
  * source array, the partial-sum rows, reduction scratch, and staging for the host-buffer
  * entry point.  From 24576 bodies on the partial rows are those of the symmetric force kernel
  * (colatus_force_plan): one row of 16 bytes per body for every source split and every block
- * distance, capped at 8 GiB -- 0.13 GB at n = 131072, 6.1 GB at 2^20, 8.9 GB at 2^22 (about
+ * distance, capped at 8 GiB -- 0.13 GB at n = 131072, 2.6 GB at 2^20, 8.9 GB at 2^22 (about
  * 1.1 KB per body below 24576).  Non-decreasing in n_max: a workspace sized for n_max serves
  * every n <= n_max.  Pure host arithmetic; 0 if n_max < 1. */
 size_t colatus_workspace_bytes(int64_t n_max);
@@ -313,7 +313,7 @@ int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 /* Which force kernel an evaluation of target_count targets out of n bodies takes (eq. 1).
  * Whole-range evaluations (target_count == n) of at least 24576 bodies use the SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
  * per unordered pair and applied to both bodies (Newton's third law) -- 16 packed FP32 operations per
- * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 1536 (1024 below 65536 bodies); block a meets the `distances`
+ * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 4096 (1024 below 65536 bodies); block a meets the `distances`
  * blocks a+1 .. a+distances (mod blocks) both ways, and itself (and the antipodal block when `blocks` is even)
  * one way.  The sums a block receives from each distance are kept as partial rows in the workspace and
  * added in fixed row order (in FP64 when there are more than 16 rows), so results are reproducible bit for
@@ -331,8 +331,8 @@ int colatus_force_plan(int64_t n, int64_t target_count, int with_potential, int6
  *   "source_splits" in [0,64] (capped at 16 above 65536 bodies and for the symmetric kernel);
  *   "symmetric": 0 = never use the symmetric kernel, 1 = automatic (default after colatus_init),
  *                2 = whenever the evaluation allows it (any n; for tests);
- *   "symmetric_block": bodies per block of the symmetric kernel, 1024 or 1536 (0 = automatic: 1024 below 65536
- *                bodies, 1536 from there on);
+ *   "symmetric_block": bodies per block of the symmetric kernel, 1024, 1536 or 4096 (0 = automatic: 1024 below
+ *                65536 bodies, 4096 from there on);
  *   "symmetric_rows": cap on the partial rows one launch of the symmetric kernel may use (0 = what the
  *                workspace holds, else >= 2): a small value splits an evaluation into several launches. */
 int colatus_set_option(const char *name, int64_t value);

@@ -37,14 +37,15 @@ constexpr int RUN_CHUNK = 1024;       // steps per coefficient-table upload in c
 constexpr int GRAPH_STEPS = COLATUS_GRAPH_STEPS;        // steps per replay of the multi-step graph (two-kernel loop; divides RUN_CHUNK)
 
 // symmetric (each pair once) force kernel, force_sym_kernels.cuh: whole-range evaluations of at least SYM_MIN_N bodies
-// Three variants: blocks of 4096 bodies (16 targets per thread, 254 registers, ONE CTA per SM, 512-source tiles) from
-// SYM_WIDE_N bodies on -- the per-source work of the source side (shuffle tree, permuted load, address arithmetic) is
+// Variants: blocks of 4096 bodies (16 targets per thread, 254 registers, ONE CTA per SM, 512-source tiles) from
+// SYM_MID_N bodies on -- the per-source work of the source side (shuffle tree, permuted load, address arithmetic) is
 // amortised over 16 targets instead of 6 and 8 independent chains per thread replace the second CTA: 292.8 ms against
-// 313.8 ms at N = 2^20 (profiles/r02_symmetric_kernel.md section 4c); blocks of 1536 (6 targets per thread, two CTAs
-// per SM) below that; and below SYM_MID_N blocks of 1024 (4 targets per thread, 256-source tiles), whose finer tiles
-// split better over the SMs (N = 32768: 32 x 14 CTAs of 4.9 tiles against 22 x 13 of 2.8; 7 % faster; section 4b)
+// 313.8 ms at N = 2^20 (profiles/r02_symmetric_kernel.md section 4c); below SYM_MID_N blocks of 1024 (4 targets per
+// thread, two CTAs per SM, 256-source tiles), whose finer tiles split better over the SMs (section 4b).  The first
+// variant written, blocks of 1536 (6 targets per thread, two CTAs per SM), is between the two everywhere (within
+// 1 % of the better one at 49152 and 98304 bodies only) and stays selectable ("symmetric_block") for comparisons.
 constexpr int64_t SYM_MID_N = 65536;
-constexpr int64_t SYM_WIDE_N = 131072;
+constexpr int64_t SYM_WIDE_N = SYM_MID_N;
 constexpr int64_t SYM_MIN_N = 24576;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
 constexpr int SYM_MAX_SPLITS = 24;
 constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)

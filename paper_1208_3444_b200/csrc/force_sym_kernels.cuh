@@ -6,7 +6,8 @@
 // receives -m_k g_kj (Newton's third law).  The one-directional kernel of force_kernels.cuh evaluates g twice;
 // this kernel evaluates it once and applies it to both bodies, for whole-range evaluations (targets = sources):
 //
-//   * bodies are cut into NB blocks of BT = 512*IP (the targets one CTA keeps in registers, as in force_kernel);
+//   * bodies are cut into NB blocks of BT = 512*IP (the targets one CTA keeps in registers, as in force_kernel;
+//     IP = 8: 16 targets per thread, 254 registers, one CTA per SM, from 65536 bodies on; IP = 2 below);
 //     block a is paired with the H = (NB-1)/2 blocks b = a+1 .. a+H (mod NB) -- a circulant half, so every block
 //     has the same amount of work and every unordered block pair is visited exactly once -- plus, one-directionally
 //     (plain tile body, reaction ignored), with itself and, when NB is even, with the antipodal block a + NB/2;

@@ -233,7 +233,7 @@ def test_plan_of_the_baseline_configurations(session):
         assert small["symmetric"] == 0
         for n in (32768, 100000, 131072, 1 << 20):
             p = B.colatus_force_plan(n)
-            block = 1024 if n < 65536 else (1536 if n < 131072 else 4096)
+            block = 1024 if n < 65536 else 4096
             assert p["symmetric"] == 1 and p["launches"] == 1 and p["blocks"] == (n + block - 1) // block
             assert p["partial_rows"] == p["splits"] + p["distances"]
         big = B.colatus_force_plan(1 << 22)
