@@ -45,9 +45,11 @@ __device__ __forceinline__ void sym_tile_body(const unsigned char *tile, const u
     // B200 (N = 2^20, % of peak by the 20-flop convention): eight per-lane byte offsets (p ^ f) * 16 kept in registers
     // (equal-mass body: 104.4 against 102.8), or the lane's row pointer plus a per-bit signed offset -- p ^ f =
     // f + sum over the set bits b of p of (f has b ? -b : +b) -- which needs no extra registers (general body:
-    // 94.2 against 91.5); the first formulation, ((jb + p) ^ f) << 4 computed per load, gave 92.9 / 101.4.
+    // 94.2 against 91.5); the first formulation, ((jb + p) ^ f) << 4 computed per load, gave 92.9 / 101.4.  With 16
+    // targets per thread (IP = 8) the registers are gone and the row-pointer form wins for equal masses too
+    // (265.7 against 267.1 ms).
     int q[8];
-    if (EQM) {
+    if (EQM && IP <= 3) {
 #pragma unroll
         for (int p = 0; p < 8; ++p) q[p] = (p << 4) ^ (f << 4);
     }
@@ -58,8 +60,8 @@ __device__ __forceinline__ void sym_tile_body(const unsigned char *tile, const u
         for (int p = 0; p < 8; ++p) {
             const int off = ((p & 1) ? ((f & 1) ? -16 : 16) : 0) + ((p & 2) ? ((f & 2) ? -32 : 32) : 0) +
                             ((p & 4) ? ((f & 4) ? -64 : 64) : 0);
-            const float4 S = EQM ? *reinterpret_cast<const float4 *>(tile + (jb << 4) + q[p])
-                                 : *reinterpret_cast<const float4 *>(row + off);
+            const float4 S = (EQM && IP <= 3) ? *reinterpret_cast<const float4 *>(tile + (jb << 4) + q[p])
+                                              : *reinterpret_cast<const float4 *>(row + off);
             const u64 X = pack2(S.x, S.x), Y = pack2(S.y, S.y), Z = pack2(S.z, S.z), M = pack2(S.w, S.w);
             u64 rx = 0ull, ry = 0ull, rz = 0ull;
 #pragma unroll
