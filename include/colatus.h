@@ -328,7 +328,8 @@ int colatus_force_plan(int64_t n, int64_t target_count, int with_potential, int6
 
 /* Tuning overrides for measurements (0 restores the automatic choice):
  *   "targets_per_thread" in {0,2,4,6} (non-zero also selects the one-directional kernel);
- *   "source_splits" in [0,64] (capped at 16 above 65536 bodies and for the symmetric kernel);
+ *   "source_splits" in [0,64] (capped at 16 above 65536 bodies; for the symmetric kernel at 32, 16 and 24 with
+ *                blocks of 1024, 1536 and 4096 bodies);
  *   "symmetric": 0 = never use the symmetric kernel, 1 = automatic (default after colatus_init),
  *                2 = whenever the evaluation allows it (any n; for tests);
  *   "symmetric_block": bodies per block of the symmetric kernel, 1024, 1536 or 4096 (0 = automatic: 1024 below

@@ -47,7 +47,7 @@ constexpr int GRAPH_STEPS = COLATUS_GRAPH_STEPS;        // steps per replay of t
 constexpr int64_t SYM_MID_N = 65536;
 constexpr int64_t SYM_WIDE_N = SYM_MID_N;
 constexpr int64_t SYM_MIN_N = 24576;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
-constexpr int SYM_MAX_SPLITS = 24;
+constexpr int SYM_MAX_SPLITS = 32;
 constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)
 constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch can always hold
 constexpr size_t SYM_ROWS_BUDGET = (size_t)8 << 30;               // bytes of partial rows before an evaluation is chunked
@@ -280,9 +280,11 @@ Geometry choose_sym_geometry(int64_t n, int part = 0, int parts = 1, bool potent
     }
     const int tpb = geo.tpb();
     const double plain_tiles = tpb * ((geo.nb & 1) ? 1.0 : 2.0) * 0.68;   // a one-directional tile costs ~0.68 symmetric ones
-    const double c0 = geo.IP == 3 ? 0.04 : 0.12;                           // per-CTA overhead in units of one tile
+    const double c0 = geo.IP == 2 ? 0.05 : 0.04;                           // per-CTA overhead in units of one tile
     double best_cost = -1.0;
-    const int smax = geo.IP > 3 ? SYM_MAX_SPLITS : 16;     // one CTA per SM: the wave count is coarser, more splits help
+    // more splits than the 16 of the first variant help where the wave count is coarse (one CTA per SM: up to 24) and
+    // where a block has few tiles (1024-body blocks: up to 32; N = 32768: kernel 0.335 ms with 32 against 0.363 with 14)
+    const int smax = geo.IP > 3 ? 24 : (geo.IP == 2 ? SYM_MAX_SPLITS : 16);
     for (int s = 1; s <= smax; ++s) {
         if (g.force_splits && g.force_splits <= smax && g.force_splits < rows_avail && s != g.force_splits)
             continue;

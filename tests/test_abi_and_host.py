@@ -68,9 +68,9 @@ def test_workspace_bytes_is_host_arithmetic():
     # below 24576 bodies: staged copy + 64 split partials + scratch: ~1.1 KB per body
     w4k = B.colatus_workspace_bytes(4096)
     assert w4k % 256 == 0 and 64 * 16 * 4096 < w4k < 8 * (1 << 20)
-    # symmetric kernel (colatus_force_plan): (24 + 127) partial rows of 256 x 4096 bodies at 2^20 ...
+    # symmetric kernel (colatus_force_plan): (32 + 127) partial rows of 256 x 4096 bodies at 2^20 ...
     w20, w22 = B.colatus_workspace_bytes(1 << 20), B.colatus_workspace_bytes(1 << 22)
-    rows20 = (24 + 127) * 256 * 4096 * 16
+    rows20 = (32 + 127) * 256 * 4096 * 16
     assert w20 % 256 == 0 and rows20 < w20 < rows20 + 100 * (1 << 20)
     # ... capped at 8 GiB of rows (the evaluation is then chunked over block distances)
     assert (8 << 30) < w22 < (8 << 30) + 400 * (1 << 20)
