@@ -16,7 +16,7 @@ same workload; it is a deliberately slow baseline, not the target.
 
 N > 1 (one rank per GPU): bodies owned in slices, positions all-gathered over NCCL once per step after the first
 drift; eq. (1) divided by block pairs (symmetric evaluation: every rank evaluates its share of the unordered pairs,
-one all-reduce of the float4[n] partial forces) or, below 24576 bodies, by targets; diagnostics by one all-reduce;
+one all-reduce of the float4[n] partial forces) or, below 20480 bodies, by targets; diagnostics by one all-reduce;
 total work fixed -> "scaling": "strong".  Under torchrun the ranks come from the environment; a plain `python bench.py --gpus N`
 re-launches itself under torch.distributed.run with N ranks (and fails loudly if fewer GPUs are visible).
 """

@@ -84,10 +84,10 @@ typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosm
 
 /* Bytes of device workspace needed for problems up to n_max bodies: the staged (padded)
  * source array, the partial-sum rows, reduction scratch, and staging for the host-buffer
- * entry point.  From 24576 bodies on the partial rows are those of the symmetric force kernel
+ * entry point.  From 20480 bodies on the partial rows are those of the symmetric force kernel
  * (colatus_force_plan): one row of 16 bytes per body for every source split and every block
  * distance, capped at 8 GiB -- 0.13 GB at n = 131072, 2.6 GB at 2^20, 8.9 GB at 2^22 (about
- * 1.1 KB per body below 24576).  Non-decreasing in n_max: a workspace sized for n_max serves
+ * 1.1 KB per body below 20480).  Non-decreasing in n_max: a workspace sized for n_max serves
  * every n <= n_max.  Pure host arithmetic; 0 if n_max < 1. */
 size_t colatus_workspace_bytes(int64_t n_max);
 
@@ -103,7 +103,7 @@ void colatus_shutdown(void);
  *                branched around (reading G4): it is m_k eps2^-1.5 * 0 = 0 exactly, PROVIDED m_k eps2^-1.5 is
  *                finite in FP32 -- the caller keeps |m| * eps2^-1.5 < 3e38 (at the floor: |m| < 3e2), else
  *                that target's force is NaN.  The same bound keeps close distinct pairs finite.
- * Whole-range evaluations of >= 24576 bodies evaluate every pair once and apply it to both bodies
+ * Whole-range evaluations of >= 20480 bodies evaluate every pair once and apply it to both bodies
  * (the symmetric kernel, colatus_force_plan); results agree with the one-directional kernel to FP32
  * summation rounding, and either is bitwise reproducible from run to run.
  * Enqueues on cuda_stream and returns without synchronising.  n in [1, 2^31-1];
@@ -311,7 +311,7 @@ int64_t  colatus_launch_count(void);
 int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
 
 /* Which force kernel an evaluation of target_count targets out of n bodies takes (eq. 1).
- * Whole-range evaluations (target_count == n) of at least 24576 bodies use the SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
+ * Whole-range evaluations (target_count == n) of at least 20480 bodies use the SYMMETRIC kernel: the pair term (x_j - x_k)/(r^2 + eps^2)^{3/2} is antisymmetric, so it is evaluated once
  * per unordered pair and applied to both bodies (Newton's third law) -- 16 packed FP32 operations per
  * 4 pair-interactions instead of 24.  Bodies are cut into blocks of 4096 (1024 below 65536 bodies); block a meets the `distances`
  * blocks a+1 .. a+distances (mod blocks) both ways, and itself (and the antipodal block when `blocks` is even)

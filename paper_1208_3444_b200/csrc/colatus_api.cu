@@ -46,7 +46,7 @@ constexpr int GRAPH_STEPS = COLATUS_GRAPH_STEPS;        // steps per replay of t
 // 1 % of the better one at 49152 and 98304 bodies only) and stays selectable ("symmetric_block") for comparisons.
 constexpr int64_t SYM_MID_N = 65536;
 constexpr int64_t SYM_WIDE_N = SYM_MID_N;
-constexpr int64_t SYM_MIN_N = 24576;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
+constexpr int64_t SYM_MIN_N = 20480;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
 constexpr int SYM_MAX_SPLITS = 32;
 constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)
 constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch can always hold

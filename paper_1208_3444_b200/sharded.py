@@ -34,7 +34,7 @@ import torch
 import torch.distributed as dist
 
 
-SYMMETRIC_MIN_N = 24576          # as libcolatus: below, the one-directional kernel on target slices is faster
+SYMMETRIC_MIN_N = 20480          # as libcolatus: below, the one-directional kernel on target slices is faster
 
 
 def partition(n: int, world: int, rank: int):

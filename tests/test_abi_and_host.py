@@ -65,7 +65,7 @@ def test_product_never_imports_oracle():
 def test_workspace_bytes_is_host_arithmetic():
     assert B.colatus_workspace_bytes(0) == 0
     assert B.colatus_workspace_bytes(-5) == 0
-    # below 24576 bodies: staged copy + 64 split partials + scratch: ~1.1 KB per body
+    # below 20480 bodies: staged copy + 64 split partials + scratch: ~1.1 KB per body
     w4k = B.colatus_workspace_bytes(4096)
     assert w4k % 256 == 0 and 64 * 16 * 4096 < w4k < 8 * (1 << 20)
     # symmetric kernel (colatus_force_plan): (32 + 127) partial rows of 256 x 4096 bodies at 2^20 ...
@@ -75,7 +75,7 @@ def test_workspace_bytes_is_host_arithmetic():
     # ... capped at 8 GiB of rows (the evaluation is then chunked over block distances)
     assert (8 << 30) < w22 < (8 << 30) + 400 * (1 << 20)
     # non-decreasing in n: a workspace sized for n_max serves every n <= n_max
-    sizes = [B.colatus_workspace_bytes(n) for n in (1, 100, 4096, 24575, 24576, 32768, 65535, 65536, 131071, 131072, 200000, 1 << 20, 1500000, 1 << 22)]
+    sizes = [B.colatus_workspace_bytes(n) for n in (1, 100, 4096, 20479, 20480, 24576, 32768, 65535, 65536, 131071, 131072, 200000, 1 << 20, 1500000, 1 << 22)]
     assert all(a <= b for a, b in zip(sizes, sizes[1:]))
 
 

@@ -1,6 +1,6 @@
 """The symmetric force kernel (every pair once, Newton's third law; force_sym_kernels.cuh, colatus_force_plan)
 against the FP64 oracle, through the C ABI.  It is picked automatically for whole-range evaluations of at least
-24576 bodies (configs 2-5: covered at full size in test_gpu_forces.py); here it is forced on at small and ragged
+20480 bodies (configs 2-5: covered at full size in test_gpu_forces.py); here it is forced on at small and ragged
 sizes so that every structural case is hit: 1 block (diagonal only), 2 blocks (antipodal only), odd and even
 block counts, ragged last blocks, every split count, equal and general masses, chunked evaluations.
 Tolerances: north_star's (G17), as in test_gpu_forces.py."""
