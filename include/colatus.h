@@ -22,7 +22,8 @@
  *   - `*_dev` pointers are DEVICE pointers owned by the caller; `*_host`
  *     pointers are host pointers owned by the caller.  The library never
  *     allocates or frees device memory: scratch comes from the caller's
- *     workspace (colatus_workspace_bytes).  It keeps raw pointers only between
+ *     workspace (colatus_workspace_bytes) -- or, for colatus_forces_static alone, from an
+ *     array built into the library.  It keeps raw pointers only between
  *     colatus_upload / colatus_trace and colatus_shutdown.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - One implicit process-wide context (one GPU per process).  Calls are not
@@ -139,6 +140,34 @@ int colatus_forces_symmetric_part(const void *pos_mass_dev, int64_t n, float eps
  * (NULL = default).  This is the end-to-end call bench.py's "e2e" times. */
 int colatus_forces_host(const float *pos_mass_host, int64_t n, float eps2, float *acc_out_host,
                         void *cuda_stream);
+
+/* ---- eq. (1), for callers who cannot allocate device memory ----------------
+ * colatus_forces needs a workspace, and a workspace is something somebody cudaMalloc'ed.  Not every caller can do
+ * that: code running inside an application whose own memory pool already owns the device memory, a callback or
+ * control loop that must not hit cudaMalloc's device-wide synchronisation (or its late out-of-memory failure), a
+ * process held to a fixed device-memory budget.  This ONE entry point serves them: it needs neither colatus_init
+ * nor a workspace, and it calls no cudaMalloc, cudaFree or any other allocating routine.  Its scratch (staged
+ * sources, source-split partial sums, the equal-mass flag) is an array built into the library's device image --
+ * about 4.5 MiB, which every GPU that loads this library's kernels holds until the process exits, whether or not
+ * this function is ever called.  That is the reason for the modest limit:
+ *     1 <= n <= COLATUS_STATIC_MAX_N  (32768 = 32^3, the largest run of the paper);
+ * larger n is refused with COLATUS_INVALID_ARG and a message naming the limit (use colatus_forces then).
+ * pos_mass_dev : const float4[n] (x, y, z, m), acc_out_dev : float4[n] (F_x, F_y, F_z, 0) -- device memory the
+ * caller already owns, 16-byte aligned, distinct; eps2 as for colatus_forces; G = the constant of eq. (1), finite
+ * (there is no context to take it from).  Same kernels and arithmetic as colatus_forces' one-directional path with
+ * a fixed geometry (2 targets per thread, up to 16 source splits -- a pure function of n and the SM count), so
+ * results agree with colatus_forces to FP32 summation rounding and repeat bit for bit from call to call.  The
+ * eq. (10) source and the background term of colatus_set_deformation / _background are NOT added.
+ * Runs on the CURRENT device (cudaGetDevice); enqueues on cuda_stream and returns without synchronising.
+ * The first call on each device also does a one-time set-up (looks up the array's device address and the SM
+ * count, which may make the driver load the library's device code): make that first call outside any stream
+ * capture.  All calls share the one array, and it keeps what the last call left -- the function clears the
+ * one word that has to start at zero itself -- so two calls whose work overlaps on the GPU (different streams,
+ * no ordering between them) race; order them on one stream or with events.  Independent of the workspace: it
+ * may be mixed freely with the other entry points.  Not thread-safe, like the rest of the library. */
+#define COLATUS_STATIC_MAX_N 32768
+int colatus_forces_static(const void *pos_mass_dev, int64_t n, float eps2, double G, void *acc_out_dev,
+                          void *cuda_stream);
 
 /* ---- eqs. (3)-(5): resident simulation state ----------------------------------------
  * Binds caller-owned device buffers (float4[n] each); all later step work is enqueued

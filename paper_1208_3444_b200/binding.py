@@ -48,6 +48,7 @@ SIGNATURES = {
     "colatus_forces_potential": (c_int, [c_void_p, c_int64, c_float, c_void_p, c_void_p]),
     "colatus_forces_range": (c_int, [c_void_p, c_int64, c_int64, c_int64, c_float, c_void_p, c_void_p]),
     "colatus_forces_host": (c_int, [c_void_p, c_int64, c_float, c_void_p, c_void_p]),
+    "colatus_forces_static": (c_int, [c_void_p, c_int64, c_float, c_double, c_void_p, c_void_p]),
     "colatus_upload": (c_int, [c_void_p, c_void_p, c_void_p, c_int64, c_float, c_void_p]),
     "colatus_step": (c_int, [c_double, c_double, c_double]),
     "colatus_step_coefficients": (c_int, [c_double, c_double, c_double, POINTER(c_double)]),
@@ -176,6 +177,16 @@ def colatus_forces_host(pos_mass_host, n, eps2, acc_out_host, stream=None):
     """Host buffers: numpy float32 arrays or pinned torch CPU tensors of shape [n,4]."""
     _check(lib().colatus_forces_host(_host_ptr(pos_mass_host), int(n), float(eps2), _host_ptr(acc_out_host),
                                      _stream(stream)))
+
+
+STATIC_MAX_N = 32768          # COLATUS_STATIC_MAX_N of include/colatus.h
+
+
+def colatus_forces_static(pos_mass, n, eps2, G, acc_out, stream=None):
+    """Eq. (1) for callers who cannot cudaMalloc a workspace (a plug-in under another allocator, a loop that must
+    not synchronise the device): scratch lives in an array inside libcolatus, so n <= STATIC_MAX_N.  Needs no
+    colatus_init; runs on the current device.  Calls share that array: keep them ordered on the GPU."""
+    _check(lib().colatus_forces_static(_ptr(pos_mass), int(n), float(eps2), float(G), _ptr(acc_out), _stream(stream)))
 
 
 def _host_ptr(a):

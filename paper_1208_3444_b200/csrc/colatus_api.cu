@@ -1470,3 +1470,126 @@ int colatus_set_option(const char *name, int64_t value) {
 const char *colatus_last_error(void) { return g.err; }
 
 }  // extern "C"
+
+// ================================================================================================
+// colatus_forces_static: eq. (1), for callers who have no device memory to give as a workspace.
+//
+// Every other entry point takes its scratch (staged sources, source-split partial sums, the equal-mass flag) from the
+// workspace handed to colatus_init, which somebody had to cudaMalloc.  Some callers cannot: a plug-in running inside a
+// host application whose own pool already owns the device memory, a callback or a tight control loop where a
+// cudaMalloc (it synchronises the whole device and may fail late) is not acceptable, a process started with a fixed
+// device-memory budget.  For them the same three kernels run here with their scratch in the file-scope device array
+// below.  The array is part of the library's image: every GPU on which this library's module gets loaded sets
+// COLATUS_STATIC_BYTES (4.5 MiB) aside until the process exits, used or not -- which is why the limit is modest.
+//
+// `static_scratch` is a device symbol.  In HOST code the name stands for a host-side shadow of it, not for a device
+// address: a kernel handed `static_scratch` (or &static_scratch[0]) from host code would fault or, on a system whose
+// GPU can reach host memory, quietly work on the wrong memory.  The device address is asked for once per device,
+// with that device current, through cudaGetSymbolAddress, in this file (the symbol has file scope), and that pointer
+// is what the kernels get.
+namespace {
+
+constexpr int64_t STATIC_MAX_N = COLATUS_STATIC_MAX_N;
+constexpr int STATIC_TJ = 128;                        // force_kernel<1, 128, ...>: 512 targets per CTA, 128-source tiles
+constexpr int STATIC_MAX_SPLITS = 16;                 // as the automatic choice of the workspace path: FP32 row sums
+constexpr size_t STATIC_FLAG_BYTES = 256;
+constexpr size_t STATIC_STAGED_BYTES = (size_t)(STATIC_MAX_N + STATIC_MAX_SPLITS * STATIC_TJ) * 16;
+constexpr size_t STATIC_PARTIAL_CELLS = (size_t)8 * STATIC_MAX_N;   // float4 cells of partial sums: splits * n <= this
+constexpr size_t COLATUS_STATIC_BYTES = STATIC_FLAG_BYTES + STATIC_STAGED_BYTES + STATIC_PARTIAL_CELLS * 16;
+constexpr int STATIC_MAX_DEVICES = 64;
+
+static __device__ __align__(256) unsigned char static_scratch[COLATUS_STATIC_BYTES];
+
+struct StaticDevice {
+    bool ready = false;
+    unsigned char *base = nullptr;   // device address of static_scratch on this device
+    int sm_count = 0;
+};
+StaticDevice static_dev[STATIC_MAX_DEVICES];
+
+// Once per device, with that device current: the device address of the scratch array and the SM count.
+int static_setup(int device, StaticDevice **out) {
+    if (device < 0 || device >= STATIC_MAX_DEVICES)
+        return fail(COLATUS_INVALID_ARG, "colatus_forces_static: device ordinal %d outside [0, %d)", device,
+                    STATIC_MAX_DEVICES);
+    StaticDevice &d = static_dev[device];
+    if (!d.ready) {
+        int major = 0, sms = 0;
+        CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+        if (major != 10)
+            return fail(COLATUS_UNSUPPORTED_DEVICE, "device %d is cc %d.x; libcolatus is built for sm_100a only", device,
+                        major);
+        CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+        void *p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u))
+            return fail(COLATUS_CUDA_ERROR, "colatus_forces_static: scratch symbol resolved to %p", p);
+        d.base = static_cast<unsigned char *>(p);
+        d.sm_count = sms;
+        d.ready = true;
+    }
+    *out = &d;
+    return COLATUS_OK;
+}
+
+}  // namespace
+
+extern "C" int colatus_forces_static(const void *pos_mass_dev, int64_t n, float eps2, double G, void *acc_out_dev,
+                                     void *cuda_stream) {
+    if (!pos_mass_dev || !acc_out_dev) return fail(COLATUS_INVALID_ARG, "null pointer");
+    if (n < 1) return fail(COLATUS_INVALID_ARG, "n=%lld is below 1", (long long)n);
+    if (n > STATIC_MAX_N)
+        return fail(COLATUS_INVALID_ARG,
+                    "colatus_forces_static: n=%lld exceeds COLATUS_STATIC_MAX_N=%lld, the size its built-in scratch "
+                    "array is laid out for; larger problems need colatus_init with a workspace and colatus_forces",
+                    (long long)n, (long long)STATIC_MAX_N);
+    if (!aligned16(pos_mass_dev) || !aligned16(acc_out_dev)) return fail(COLATUS_INVALID_ARG, "pointer not 16-byte aligned");
+    if (pos_mass_dev == acc_out_dev) return fail(COLATUS_INVALID_ARG, "pos_mass and acc_out alias");
+    if (!eps2_ok(eps2)) return fail(COLATUS_INVALID_ARG, "eps2 must be finite and >= 1e-24");
+    if (!std::isfinite(G)) return fail(COLATUS_INVALID_ARG, "G is not finite");
+    int device = -1;
+    CUDA_TRY(cudaGetDevice(&device));
+    StaticDevice *d = nullptr;
+    if (int rc = static_setup(device, &d)) return rc;
+
+    // geometry: a pure function of (n, SM count), so the summation order -- and the bits -- repeat from call to call.
+    // Enough source splits for two CTAs per SM, bounded by the partial-sum cells the array holds.
+    const int64_t tiles_t = (n + 2 * FORCE_THREADS - 1) / (2 * FORCE_THREADS);
+    const int64_t src_tiles = (n + STATIC_TJ - 1) / STATIC_TJ;
+    int64_t splits = (2 * (int64_t)d->sm_count + tiles_t - 1) / tiles_t;
+    if (splits > STATIC_MAX_SPLITS) splits = STATIC_MAX_SPLITS;
+    if (splits > src_tiles) splits = src_tiles;
+    if (splits > (int64_t)(STATIC_PARTIAL_CELLS / (size_t)n)) splits = (int64_t)(STATIC_PARTIAL_CELLS / (size_t)n);
+    const int64_t tiles_per_split = (src_tiles + splits - 1) / splits;
+    const int64_t n_pad = splits * tiles_per_split * STATIC_TJ;
+    if ((size_t)n_pad * 16 > STATIC_STAGED_BYTES || (size_t)splits * (size_t)n > STATIC_PARTIAL_CELLS)
+        return fail(COLATUS_INVALID_ARG, "colatus_forces_static: internal layout overflow at n=%lld", (long long)n);
+
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int *mass_flag = reinterpret_cast<int *>(d->base);
+    float4 *staged = reinterpret_cast<float4 *>(d->base + STATIC_FLAG_BYTES);
+    float4 *partials = reinterpret_cast<float4 *>(d->base + STATIC_FLAG_BYTES + STATIC_STAGED_BYTES);
+    const float4 *pos_mass = static_cast<const float4 *>(pos_mass_dev);
+    float4 *out = static_cast<float4 *>(acc_out_dev);
+
+    // The array still holds what the previous call left.  Only the equal-mass flag has to start from zero (the staging
+    // kernel stamps it when some mass differs from body 0's); the staged sources and every partial-sum cell the
+    // reduction reads are written anew by this call's kernels.
+    constexpr int generation = 1;
+    CUDA_TRY(cudaMemsetAsync(mass_flag, 0, sizeof(int), st));
+    stage_sources_kernel<<<(unsigned)((n_pad + 255) / 256), 256, 0, st>>>(pos_mass, n, n_pad, staged, mass_flag, generation);
+    CUDA_TRY(cudaGetLastError());
+    const bool single = splits == 1;
+    CUDA_TRY(launch_ex(force_kernel<1, STATIC_TJ, NSTAGES, false, 2>, dim3((unsigned)tiles_t, (unsigned)splits),
+                       dim3(FORCE_THREADS), force_smem_bytes<1, STATIC_TJ, NSTAGES, false>(), st, false, pos_mass,
+                       (const float4 *)staged, (int64_t)0, n, (int)tiles_per_split, eps2, single ? (float)G : 1.0f,
+                       single ? 1 : 0, single ? out : partials, n, (const int *)mass_flag, generation, (int *)nullptr));
+    g.launches += 2;
+    if (!single) {
+        reduce_partials_kernel<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(partials, n, (int)splits, n, (float)G,
+                                                                                  eps2, pos_mass, 0, out);
+        CUDA_TRY(cudaGetLastError());
+        g.launches++;
+    }
+    return COLATUS_OK;
+}

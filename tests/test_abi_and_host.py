@@ -87,6 +87,16 @@ def test_uninitialised_calls_fail_loudly_without_a_device():
         B.colatus_diagnostics(1.0)
 
 
+def test_static_entry_point_limit_and_argument_checks_need_no_device():
+    """colatus_forces_static (the entry point for callers who cannot allocate a workspace): the binding's limit is
+    the header's, and the argument checks come before any CUDA call."""
+    header = open(os.path.join(ROOT, "include", "colatus.h")).read()
+    assert int(re.search(r"#define\s+COLATUS_STATIC_MAX_N\s+(\d+)", header).group(1)) == B.STATIC_MAX_N
+    assert B.lib().colatus_forces_static(None, 10, 1e-4, 1.0, None, None) == B.INVALID_ARG
+    assert B.lib().colatus_forces_static(16, B.STATIC_MAX_N + 1, 1e-4, 1.0, 32, None) == B.INVALID_ARG
+    assert "COLATUS_STATIC_MAX_N" in B.colatus_last_error()
+
+
 def test_step_coefficients_worked_example():
     """tests/golden/one_step_worked.txt: tau=1/4, a=1/2, H=4/3 -> cv = 1/2, ck = 3/2."""
     d1, cv, ck, d2 = B.colatus_step_coefficients(0.25, 0.5, 4.0 / 3.0)
