@@ -40,8 +40,13 @@
  *   - There is no CPU fallback: without an sm_100 device colatus_init returns
  *     COLATUS_UNSUPPORTED_DEVICE or COLATUS_CUDA_ERROR.
  *   - Device data are not scanned: NaN/Inf inputs give NaN outputs, not errors.
- *   - Results are bit-reproducible run to run for a fixed (n, device, build):
- *     no floating-point atomics anywhere.
+ *   - Results of every call of this library are bit-reproducible run to run for a fixed
+ *     (n, device, build, options): no floating-point atomics anywhere, all sums in a fixed order.
+ *     That is a statement about ONE GPU.  Across GPUs (paper_1208_3444_b200/sharded.py) it carries
+ *     over to target sharding, whose only exchange is an all-gather of positions (bits are moved,
+ *     not added); in symmetric sharding the shares of colatus_forces_symmetric_part are summed by
+ *     an FP32 all-reduce whose order belongs to the communication library, so forces there are
+ *     reproducible only up to that summation order (never run on more than one GPU so far).
  *   - Equal masses are detected on the device at every force evaluation (all m_j equal to
  *     m_0 in value): the kernel then applies the common mass once to the finished sums instead
  *     of once per pair (one rounding fewer per term).  No flag, no host round trip; a NaN or a
@@ -131,6 +136,8 @@ int colatus_forces_range(const void *pos_mass_dev, int64_t n, int64_t target_beg
  * single evaluation of every pair -- every GPU holds all positions (one all-gather per step, as for target sharding),
  * evaluates share `rank` of `world`, and ONE all-reduce of the float4[n] outputs gives every GPU the forces
  * (paper_1208_3444_b200/sharded.py).  Any n for which the workspace holds two partial rows (else INVALID_ARG).
+ * The eq. (10) source and the background term are NOT part of a share (they would be counted `parts` times): a
+ * driver adds them once to the summed forces with colatus_add_external.
  * Same argument rules as colatus_forces; enqueues on cuda_stream. */
 int colatus_forces_symmetric_part(const void *pos_mass_dev, int64_t n, float eps2, int part, int parts,
                                   void *acc_out_dev, void *cuda_stream);
@@ -241,7 +248,10 @@ int colatus_step_symplectic(const struct colatus_cosmo *c, double a0, double tau
  * position": every force this library returns or uses gains
  *   F_k += S (x_psi - x_k) / (|x_k - x_psi|^2 + eps^2)^{3/2}
  * (attractive for S > 0; S is NOT multiplied by G, as in eq. (10)).  S = 0 disables (default).
- * The term is not part of acc.w / W.  Applies to colatus_forces*, colatus_step* alike.  Host call. */
+ * The term is not part of acc.w / W.  Applies to colatus_forces, _potential, _range, _host, colatus_step*, colatus_run*
+ * and colatus_force_kick_drift alike; the two calls that handle caller-assembled forces -- colatus_forces_symmetric_part
+ * (a share) and colatus_kick_drift (forces as given) -- leave it to colatus_add_external, and colatus_forces_static
+ * (no context) never adds it.  Host call. */
 int colatus_set_deformation(const double x_psi[3], double strength);
 
 /* Mean-density background term (reading G22; the paper states periodic/homogeneous
@@ -267,6 +277,15 @@ int colatus_force_kick_drift(double cv, double ck, double d2);
  * step counter + 1.  This is the second half of colatus_force_kick_drift for drivers that assemble F themselves
  * (the sharded symmetric evaluation: colatus_forces_symmetric_part on every GPU, one all-reduce).  Asynchronous. */
 int colatus_kick_drift(const void *acc_dev, double cv, double ck, double d2);
+/* The external terms for forces the caller assembled itself.  colatus_forces_symmetric_part returns SHARES of
+ * eq. (1) that are summed over GPUs, so it cannot add the eq. (10) source or the
+ * background term -- they would be counted once per share -- and colatus_kick_drift takes its forces as given.  This
+ * call adds both terms, as set by colatus_set_deformation / colatus_set_background, ONCE to acc_dev = float4[target_count]
+ * (forces of the resident target range's bodies, indexed from the range's first body) at the resident positions: the
+ * sharded symmetric driver calls it between its all-reduce and colatus_kick_drift.  Nothing is launched when both terms
+ * are off.  Do not apply it to the output of colatus_forces / _range (those already contain the terms).  Asynchronous
+ * on the resident stream. */
+int colatus_add_external(void *acc_dev);
 
 /* ---- tracers -------------------------------------------------
  * After each step the velocities v^{n+1} of the k particles idx_dev[0..k) are written to

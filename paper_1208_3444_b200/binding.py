@@ -63,6 +63,7 @@ SIGNATURES = {
     "colatus_drift": (c_int, [c_double]),
     "colatus_force_kick_drift": (c_int, [c_double, c_double, c_double]),
     "colatus_kick_drift": (c_int, [c_void_p, c_double, c_double, c_double]),
+    "colatus_add_external": (c_int, [c_void_p]),
     "colatus_forces_symmetric_part": (c_int, [c_void_p, c_int64, c_float, c_int, c_int, c_void_p, c_void_p]),
     "colatus_trace": (c_int, [c_void_p, c_int, c_void_p, c_int]),
     "colatus_trace_read": (c_int, [c_void_p, c_int64, c_int]),
@@ -272,6 +273,11 @@ def colatus_force_kick_drift(cv, ck, d2):
 
 def colatus_kick_drift(acc, cv, ck, d2):
     _check(lib().colatus_kick_drift(_ptr(acc), float(cv), float(ck), float(d2)))
+
+
+def colatus_add_external(acc):
+    """Adds the eq. (10) source / background term once to caller-assembled forces of the resident target range."""
+    _check(lib().colatus_add_external(_ptr(acc)))
 
 
 def colatus_trace(idx, k, ring, capacity_steps):

@@ -462,6 +462,19 @@ struct FusedStep {
     Geometry geo;              // out: the geometry used (n_pad for the tail/head kernel's grid)
 };
 
+// eq. (10) source and mean-density background (colatus_set_deformation / _background): O(n) epilogue on finished
+// forces `out` = float4[t_count] of the targets [t_begin, t_begin + t_count).  Nothing is launched when both are off.
+int enqueue_external(const float4 *pos_mass, int64_t t_begin, int64_t t_count, float eps2, float4 *out, cudaStream_t st) {
+    if (g.def_S == 0.0 && g.bg_rho == 0.0) return COLATUS_OK;
+    const double B = (4.0 * 3.14159265358979323846 / 3.0) * g.G * g.bg_rho;
+    external_field_kernel<<<(unsigned)((t_count + 255) / 256), 256, 0, st>>>(
+        pos_mass, t_begin, t_count, out, (float)g.def_S, (float)g.def_x[0], (float)g.def_x[1], (float)g.def_x[2], eps2,
+        (float)B, (float)g.bg_c[0], (float)g.bg_c[1], (float)g.bg_c[2]);
+    CUDA_TRY(cudaGetLastError());
+    g.launches++;
+    return COLATUS_OK;
+}
+
 int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_count, float eps2, float4 *out,
                bool potential, cudaStream_t st, FusedStep *fused = nullptr) {
     const Workspace w = workspace_layout(n);
@@ -573,15 +586,7 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
             g.launches++;
         }
     }
-    if (g.def_S != 0.0 || g.bg_rho != 0.0) {   // eq. (10) / background: O(n) epilogue on the finished forces
-        const double B = (4.0 * 3.14159265358979323846 / 3.0) * g.G * g.bg_rho;
-        external_field_kernel<<<(unsigned)((t_count + 255) / 256), 256, 0, st>>>(
-            pos_mass, t_begin, t_count, out, (float)g.def_S, (float)g.def_x[0], (float)g.def_x[1], (float)g.def_x[2],
-            eps2, (float)B, (float)g.bg_c[0], (float)g.bg_c[1], (float)g.bg_c[2]);
-        CUDA_TRY(cudaGetLastError());
-        g.launches++;
-    }
-    return COLATUS_OK;
+    return enqueue_external(pos_mass, t_begin, t_count, eps2, out, st);
 }
 
 // One share of a symmetric evaluation: the block pairs whose target block lies in share `part` of `parts` (contiguous
@@ -1243,6 +1248,13 @@ int colatus_kick_drift(const void *acc_dev, double cv, double ck, double d2) {
     if (!std::isfinite(cv) || !std::isfinite(ck) || !std::isfinite(d2))
         return fail(COLATUS_INVALID_ARG, "non-finite step coefficient");
     return enqueue_kick_drift(static_cast<const float4 *>(acc_dev), cv, ck, d2, 0.f);
+}
+
+int colatus_add_external(void *acc_dev) {
+    if (!g.initialised) return fail(COLATUS_NOT_INITIALISED, "colatus_init has not been called");
+    if (!g.uploaded) return fail(COLATUS_NOT_UPLOADED, "colatus_upload has not been called");
+    if (!acc_dev || !aligned16(acc_dev)) return fail(COLATUS_INVALID_ARG, "acc_dev null or misaligned");
+    return enqueue_external(g.pos, g.t_begin, g.t_count, g.eps2, static_cast<float4 *>(acc_dev), g.stream);
 }
 
 int colatus_trace(const int32_t *idx_dev, int k, void *ring_dev, int capacity_steps) {

@@ -18,14 +18,16 @@ Symmetric mode (`symmetric=True`, the default from SYMMETRIC_MIN_N bodies on whe
 force step of a rank is `ops.forces_symmetric_part(rank, world, acc_full)` -- the block pairs whose target block lies
 in the rank's share, circulant pairing so every share is the same work, every pair evaluated once -- followed by ONE
 all-reduce (sum) of acc_full (16 n bytes: 16 MiB at 2^20, microseconds over NVLink against 314 ms / world of force
-work) and `ops.kick_drift(acc_full[slice], ...)`.  Per step: one all-gather of positions and one all-reduce of forces.
+work), `ops.add_external(acc_full[slice])` (the eq. (10) source and the background term, which a share cannot carry:
+once, on the sum) and `ops.kick_drift(acc_full[slice], ...)`.  Per step: one all-gather of positions and one all-reduce of forces.
 
 `ShardedStepper` holds only the host-side sequencing.  The per-slice work is done by an `ops`
 object: `LibcolatusOps` (the product: calls the C ABI) or, in tests/, a stand-in that lets the
 sequencing be checked on CPU without a GPU.  An `ops` object provides
     drift(d); force_kick_drift(cv, ck, d2); diagnostics(a, with_potential) -> 16 doubles over the slice;
     trace_rows(first_step, n_steps) -> float32 [n_steps, k, 4] of this rank's ring (optional);
-    forces_symmetric_part(part, parts, acc_full); kick_drift(acc_slice, cv, ck, d2) (optional: symmetric mode).
+    forces_symmetric_part(part, parts, acc_full); add_external(acc_slice); kick_drift(acc_slice, cv, ck, d2)
+    (optional: symmetric mode).
 """
 from __future__ import annotations
 
@@ -68,6 +70,10 @@ class LibcolatusOps:
 
     def kick_drift(self, acc_slice, cv, ck, d2):
         self.B.colatus_kick_drift(acc_slice, cv, ck, d2)
+
+    def add_external(self, acc_slice):
+        """eq. (10) source / background term, once, on the summed forces of the own slice (no launch when both are off)."""
+        self.B.colatus_add_external(acc_slice)
 
     def diagnostics(self, a, with_potential=False):
         return self.B.colatus_diagnostics(a, with_potential)
@@ -131,7 +137,10 @@ class ShardedStepper:
             if self.world > 1:
                 self.reduces += 1
                 dist.all_reduce(self.acc_full, op=dist.ReduceOp.SUM, group=self.group)
-            self.ops.kick_drift(self.acc_full[self.begin:self.begin + self.count], cv, ck, d2)
+            mine = self.acc_full[self.begin:self.begin + self.count]
+            if hasattr(self.ops, "add_external"):      # shares carry no external terms: once, after the sum
+                self.ops.add_external(mine)
+            self.ops.kick_drift(mine, cv, ck, d2)
         else:
             self.ops.force_kick_drift(cv, ck, d2)
         self.dirty = self.world > 1

@@ -211,3 +211,81 @@ def test_sharded_stepper_symmetric_mode_world1_and_two_emulated_ranks():
     vr = float(np.sqrt((v_ref[:, :3].astype(np.float64) ** 2).sum(1).mean()))
     assert np.abs(v2[:, :3] - v_ref[:, :3]).max() <= 2e-5 * vr and np.abs(x2[:, :3] - x_ref[:, :3]).max() <= 1e-6
     assert not np.array_equal(x2[:, :3], pm[:, :3])
+
+
+def test_symmetric_sharded_step_keeps_the_external_terms():
+    """ADVICE r2: a share of a symmetric evaluation carries no eq. (10) source / background term (PAPER.md:89-96;
+    they would be counted once per share), so the driver adds them ONCE after the all-reduce (colatus_add_external).
+    ShardedStepper in symmetric mode with both terms on must follow colatus_step -- which applies them inside the
+    library -- to rounding, at world size 1 and with two ranks emulated one after the other; and must differ from the
+    run without the terms (non-vacuous)."""
+    import torch
+    from paper_1208_3444_b200.harness import Session
+    from paper_1208_3444_b200.sharded import LibcolatusOps, ShardedStepper
+    cfg, pm, vel = inputs.make_config(1)
+    xpsi, S = np.array([0.5, 0.5, 1.5]), 0.5
+    cen, rho = np.array([0.5, 0.5, 0.5]), 1.0
+    steps = 10
+    mids, _ = oracle.midstep_schedule(cfg.cosmo, cfg.a_start, cfg.tau, steps)
+    half = cfg.n // 2
+    with Session(cfg.G, cfg.n) as s:
+        def single(with_terms):
+            if with_terms:
+                B.colatus_set_deformation(xpsi, S)
+                B.colatus_set_background(cen, rho)
+            s.upload(pm, vel, cfg.eps2)
+            for a, H in mids:
+                B.colatus_step(cfg.tau, a, H)
+            out = s.download()
+            B.colatus_set_deformation(None, 0.0)
+            B.colatus_set_background(None, 0.0)
+            return out
+        x_ref, v_ref = single(True)
+        x_off, v_off = single(False)
+
+        B.colatus_set_deformation(xpsi, S)
+        B.colatus_set_background(cen, rho)
+        pos, v = s.to_device(pm), s.to_device(vel)
+        stepper = ShardedStepper(pos, cfg.n, LibcolatusOps(pos, v, torch.zeros_like(pos), cfg.n, cfg.eps2, 0, cfg.n),
+                                 symmetric=True)
+        for a, H in mids:
+            stepper.step(cfg.tau, a, H)
+        torch.cuda.synchronize()
+        x1, v1 = pos.cpu().numpy(), v.cpu().numpy()
+
+        # two ranks, one after the other: shares summed (the all-reduce), external terms once per slice, kick-drift
+        pos, v = s.to_device(pm), s.to_device(vel)
+        B.colatus_upload(pos, v, torch.zeros((half, 4), dtype=torch.float32, device=pos.device), cfg.n, cfg.eps2)
+        for a, H in mids:
+            c = B.colatus_step_coefficients(cfg.tau, a, H)
+            for b in (0, half):
+                B.colatus_set_target_range(b, half)
+                B.colatus_drift(c[0])
+            parts = [torch.empty_like(pos) for _ in range(2)]
+            for r in range(2):
+                B.colatus_forces_symmetric_part(pos, cfg.n, cfg.eps2, r, 2, parts[r])
+            total = parts[0] + parts[1]
+            for b in (0, half):
+                B.colatus_set_target_range(b, half)
+                B.colatus_add_external(total[b:b + half])
+                B.colatus_kick_drift(total[b:b + half], c[1], c[2], c[3])
+        torch.cuda.synchronize()
+        x2, v2 = pos.cpu().numpy(), v.cpu().numpy()
+        B.colatus_set_deformation(None, 0.0)
+        B.colatus_set_background(None, 0.0)
+        # with both terms off nothing is launched and the forces stay as given
+        B.colatus_set_target_range(0, half)
+        before = B.colatus_launch_count()
+        B.colatus_add_external(total[:half])
+        assert B.colatus_launch_count() == before
+    vr = float(np.sqrt((v_ref[:, :3].astype(np.float64) ** 2).sum(1).mean()))
+    for xs, vs in ((x1, v1), (x2, v2)):
+        assert np.abs(vs[:, :3] - v_ref[:, :3]).max() <= 2e-4 * vr and np.abs(xs[:, :3] - x_ref[:, :3]).max() <= 5e-6
+    assert np.abs(x_off[:, :3] - x_ref[:, :3]).max() >= 1e-3              # the terms matter in this set-up
+    # and against the oracle with the same terms (readings G21 / G22; G16 bar of the 10-step trajectories)
+    st = oracle.State(pm, vel, cfg.eps2, cfg.G)
+    st.deformation, st.background = (xpsi, S), (cen, rho)
+    for a, H in mids:
+        st.step(cfg.tau, a, H)
+    for xs in (x1, x2):
+        assert np.linalg.norm(xs[:, :3].astype(np.float64) - st.x, axis=1).max() <= 1e-5

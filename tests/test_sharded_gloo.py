@@ -117,6 +117,12 @@ class OracleSliceOps:
         acc_full[:, :3] = torch.from_numpy(F)
         acc_full[:, 3] = 0.0
 
+    external_calls = 0
+
+    def add_external(self, acc_slice):
+        """Stand-in for colatus_add_external: once per step, on the summed forces of the own slice."""
+        self.external_calls += 1
+
     def kick_drift(self, acc_slice, cv, ck, d2):
         self.vel.mul_(cv).add_(ck * acc_slice[:, :3])
         s = slice(self.begin, self.begin + self.count)
@@ -149,6 +155,7 @@ def _worker(rank, world, port, pm, vel, eps2, G, coeffs, out_dir, symmetric=Fals
             stepper.step_coeffs(*c)
         assert stepper.gathers == len(coeffs) and stepper.dirty          # ONE all-gather per step
         assert stepper.reduces == (len(coeffs) if symmetric else 0)       # symmetric mode: + ONE all-reduce of forces
+        assert stepper.ops.external_calls == (len(coeffs) if symmetric else 0)   # external terms: once, after the sum
         other = slice(0, count) if rank == 1 else slice(count, 2 * count)
         stale = pos[other].clone()
         d_kin = stepper.diagnostics(0.5)                                  # no potential: no gather needed
