@@ -45,6 +45,10 @@ FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8, "sym
                              "profile": "profiles/r02_force_kernel_ncu_full.txt"}
 SYM_KERNEL_DRAM_TRAFFIC = {"bytes": 254605824 + 2335484000, "n": 1 << 20, "splits": 15,
                            "profile": "profiles/r02_force_sym_kernel_ncu_full.txt"}
+# sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active of the same captures (the hardware counter beside the
+# modelled lane-op figure)
+FORCE_KERNEL_FMA_PIPE_NCU = {"value": 0.883, "profile": "profiles/r02_force_kernel_ncu_full.txt"}
+SYM_KERNEL_FMA_PIPE_NCU = {"value": 0.837, "profile": "profiles/r02_force_sym_kernel_ncu_full.txt"}
 # executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
 # (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention
 EXECUTED_FLOP_GENERAL, EXECUTED_FLOP_EQUAL_MASS = 19.0, 18.0
@@ -76,6 +80,9 @@ def parse():
                     help="4 = N=2^20 (the reported workload, default); 5 = N=2^22 (the at-scale case of BASELINE.json); "
                          "2, 3 = the equal-mass stepping configurations (N = 32768, 131072), for profiling the equal-mass loop")
     ap.add_argument("--n", type=int, default=0, help="override N (debug only; the reported workload is 2^20)")
+    ap.add_argument("--only-step-loop", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="profiling aid: run only the colatus_run step loop of this configuration (optionally with --n) "
+                         "and print its steps/s as one JSON line -- the launches ncu captures for the small-N kernels")
     ap.add_argument("--sharded-driver", action="store_true",
                     help="run the multi-GPU step driver (sharded.py) even at N = 1: a self-test of that code path on one GPU")
     return ap.parse_args()
@@ -149,7 +156,24 @@ def oracle_sample_rate(pm, cfg, seconds_target=12.0, max_targets=65536):
     return k * n / dt / 1e9, oracle.num_threads(), f"{k} seeded targets x {n} sources (config {cfg.index}), FP64, {dt:.1f} s"
 
 
-def step_loop_rates(device_index):
+def oracle_all_pairs_rates():
+    """"oracle timing ... all pairs for configs 1-3" -- the oracle as it stands, every target of each
+    configuration, on the host cores (about 5 s in all)."""
+    import oracle
+    from paper_1208_3444_b200 import inputs
+    out = {}
+    for index in (1, 2, 3):
+        cfg, pm, _ = inputs.make_config(index)
+        t0 = time.perf_counter()
+        oracle.forces(pm, cfg.eps2, cfg.G)
+        dt = time.perf_counter() - t0
+        out[f"config{index}"] = {"n": cfg.n, "value": float(cfg.n) ** 2 / dt / 1e9, "unit": UNIT, "seconds": dt,
+                                 "cores": oracle.num_threads(), "kind": "oracle",
+                                 "sample": f"all {cfg.n} targets x {cfg.n} sources, FP64"}
+    return out
+
+
+def step_loop_rates(device_index, only=None, n_override=None):
     """Side measurement ("steps/s for configs 1-3, CUDA graph on/off"): whole leapfrog steps per
     second of the small, launch-bound configurations through colatus_run with graph replay, the same kernels
     launched one by one from the native loop, and colatus_step called per step from Python.  Device time by
@@ -160,7 +184,9 @@ def step_loop_rates(device_index):
     from paper_1208_3444_b200.harness import Session
     out = {}
     for index, steps in ((1, 400), (2, 200), (3, 40)):
-        cfg, pm, vel = inputs.make_config(index)
+        if only and index != only:
+            continue
+        cfg, pm, vel = inputs.make_config(index, n_override if only else None)
         row = {"n": cfg.n, "steps_timed": steps}
         with Session(cfg.G, cfg.n, device=device_index) as s:
             tau = 1e-3 * cfg.tau                       # tiny steps: the state stays near the initial one
@@ -208,7 +234,9 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"config {cfg.index}: N={n} clusters+background, eps={cfg.eps}", "n": n},
+        "config": {"workload": workload_text(cfg, n), "n": n, "interactions_per_step": float(n) * n,
+                   "sampled": f"each step evaluates {k} seeded targets x all {n} sources (a bounded sample of the "
+                              "workload's N^2 interactions)"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -222,6 +250,12 @@ WORKLOAD_TEXT = {4: "64 Gaussian clusters + 50% uniform background, log-normal m
                  5: "256 Gaussian clusters + 50% uniform background, log-normal masses",
                  3: "Plummer sphere + 30% uniform background, equal masses",
                  2: "32^3 lattice + Gaussian displacements, equal masses"}
+
+
+def workload_text(cfg, n):
+    """config.workload: ONE string for the native and the reference arm (the driver compares them)."""
+    return (f"config {cfg.index} ({cfg.name}): N={n}, " + WORKLOAD_TEXT[cfg.index] +
+            f", eps={cfg.eps}; one full leapfrog step + diagnostics per step")
 
 
 def relaunch_with_ranks(args):
@@ -321,12 +355,14 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
     k_ms = kernel_ms / max(kernel_launches, 1)
     per_s = pairs_per_launch / (k_ms * 1e-3)
     achieved = FLOP_PER_INTERACTION * per_s / 1e12
+    algorithmic_bytes = 32 * n
     if sym:
         cap = SYM_KERNEL_DRAM_TRAFFIC
         traffic = cap["bytes"] if (cap and n == cap["n"] and world == 1 and plan["splits"] == cap["splits"]) else None
         executed, lane_ops = sym_work(geo["targets_per_thread"], equal_mass)
-        # staged bodies read as targets and as sources, every partial row written once
-        algorithmic_bytes = 16 * plan["padded_bodies"] * (2 + plan["splits"] + plan["distances"])
+        # workspace traffic the method does not ask for: the staged copy and every partial row, written once
+        workspace_bytes_written = 16 * plan["padded_bodies"] * (1 + plan["splits"] + plan["distances"])
+        pipe_ncu = SYM_KERNEL_FMA_PIPE_NCU if traffic else None
         kernel = "force_sym_kernel<%d,%d,4,%d,%s> (every pair once, applied to both bodies)%s%s" % (
             geo["targets_per_thread"] // 2, 256 if geo["targets_per_thread"] == 4 else 512,
             1 if geo["targets_per_thread"] > 6 else 2,
@@ -340,7 +376,8 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
         traffic = cap["bytes"] if (n == cap["n"] and world == 1 and geo["source_splits"] == cap["splits"]) else None
         lane_ops = FMA_PIPE_LANE_OPS_EQUAL_MASS if equal_mass else FMA_PIPE_LANE_OPS_GENERAL
         executed = EXECUTED_FLOP_EQUAL_MASS if equal_mass else EXECUTED_FLOP_GENERAL
-        algorithmic_bytes = 16 * n * (2 + (geo["source_splits"] if geo["source_splits"] > 1 else 0))
+        workspace_bytes_written = 16 * n * (1 + (geo["source_splits"] if geo["source_splits"] > 1 else 0))
+        pipe_ncu = FORCE_KERNEL_FMA_PIPE_NCU if traffic else None
         kernel = "force_kernel<%d,%d,4,false,2>%s" % (geo["targets_per_thread"] // 2,
                                                       {6: 512, 4: 512, 2: 128}[geo["targets_per_thread"]],
                                                       " equal-mass loop" if equal_mass else "")
@@ -348,6 +385,9 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
                 "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
                 "traffic_from": cap["profile"] if traffic else None,
                 "algorithmic_bytes": algorithmic_bytes,
+                "algorithmic_bytes_basis": "SURVEY 8(d): read N bodies + write N forces = 32 N bytes per evaluation",
+                "workspace_bytes_written": workspace_bytes_written,
+                "traffic_over_algorithmic": traffic / algorithmic_bytes if traffic else None,
                 "kernel": kernel,
                 "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / ms_step,
@@ -357,11 +397,16 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
                 "frac_note": ("achieved = ALGORITHMIC flops: 20 flop x N^2 pair interactions delivered / kernel time "
                               "(BASELINE convention)." + (" The symmetric kernel evaluates each unordered pair once "
                               "and applies it to both bodies, so it EXECUTES ~13.2 flop per delivered interaction: "
-                              "frac can exceed 20/24 = 0.833, the ceiling of a one-directional kernel; "
-                              "frac_executed_flops and fma_pipe_busy_frac count what the SMs really did."
+                              "frac (= algorithmic_frac) can exceed 20/24 = 0.833, the ceiling of a one-directional "
+                              "kernel, and 1; the hardware utilisation figures are frac_executed_flops (SASS flop "
+                              "count x rate), fma_pipe_busy_frac_modelled (lane-ops x rate) and "
+                              "fma_pipe_busy_frac_ncu (sm__pipe_fma_cycles_active of the committed capture)."
                               if sym else "")),
                 "frac_executed_flops": executed * per_s / 1e12 / FP32_PEAK_TFLOPS,
-                "fma_pipe_busy_frac": lane_ops * per_s / (SM_COUNT * FP32_LANES * SM_MAX_MHZ * 1e6),
+                "fma_pipe_busy_frac_modelled": lane_ops * per_s / (SM_COUNT * FP32_LANES * SM_MAX_MHZ * 1e6),
+                "fma_pipe_busy_frac_ncu": pipe_ncu["value"] if pipe_ncu else None,
+                "fma_pipe_busy_frac_ncu_from": pipe_ncu["profile"] if pipe_ncu else None,
+                "algorithmic_frac": achieved / FP32_PEAK_TFLOPS,
                 "frac_at_sampled_clock": (achieved / (FP32_PEAK_TFLOPS * clocks["sm_mhz"] / SM_MAX_MHZ)
                                           if clocks.get("sm_mhz") else None)}
 
@@ -408,6 +453,10 @@ def run_native(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.only_step_loop:
+        print(json.dumps({"step_loops": step_loop_rates(local_rank, args.only_step_loop, args.n or None)}), flush=True)
+        return
+
     # measured denominator (register-only FMA loops of libcolatus_probe), beside the derived 74.45 TFLOP/s
     cal_ffma, _ = P.fp32_peak(False, local_rank)
     cal_ffma2, _ = P.fp32_peak(True, local_rank)
@@ -420,9 +469,12 @@ def run_native(args):
     roofline["frac_of_measured_peak"] = roofline["achieved"] / max(cal_ffma, cal_ffma2)
 
     cpu_baseline = None
+    cpu_baseline_configs = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, cores, sample = oracle_sample_rate(pm, cfg)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        if not args.n and args.config == WORKLOAD_CONFIG:
+            cpu_baseline_configs = oracle_all_pairs_rates()
 
     default_run = world == 1 and not args.n and args.config == WORKLOAD_CONFIG
     step_loops = None
@@ -445,8 +497,7 @@ def run_native(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": m["ms_step"], "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"config {cfg.index} ({cfg.name}): N={n}, " + WORKLOAD_TEXT[cfg.index] +
-                                   f", eps={cfg.eps}; one full leapfrog step + diagnostics per step",
+            "config": {"workload": workload_text(cfg, n),
                        "n": n, "interactions_per_step": float(n) * n, "tracers": N_TRACERS,
                        "parallelism": "single GPU" if world == 1 else f"eq. (1) divided over {world} GPUs (symmetric "
                                                                        "evaluation: by block pairs, one all-reduce of "
@@ -457,7 +508,8 @@ def run_native(args):
                        "geometry": m["geo"]},
             "gflops": value * FLOP_PER_INTERACTION,
             "frac_fp32_peak": value * FLOP_PER_INTERACTION / 1e3 / (FP32_PEAK_TFLOPS * world),
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": m["e2e"],
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "cpu_baseline_configs": cpu_baseline_configs,
+            "e2e": m["e2e"],
             "gpu_launches": m["launches"], "clocks": m["clocks"],
             "step_loops": step_loops, "config5": config5,
             "diagnostics_last_step": {"M": float(m["diag"][0]), "T": float(m["diag"][7])},
