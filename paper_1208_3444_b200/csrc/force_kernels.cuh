@@ -273,8 +273,8 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
     for (int i = 0; i < IP; ++i) {
         const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
         float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-        if (t < t_count) b0 = __ldg(pos_mass + t_begin + t);
-        if (t + 1 < t_count) b1 = __ldg(pos_mass + t_begin + t + 1);
+        if (t < t_count) b0 = __ldcg(pos_mass + t_begin + t);
+        if (t + 1 < t_count) b1 = __ldcg(pos_mass + t_begin + t + 1);
         nx[i] = pack2(-b0.x, -b1.x);
         ny[i] = pack2(-b0.y, -b1.y);
         nz[i] = pack2(-b0.z, -b1.z);
@@ -291,9 +291,9 @@ force_kernel(const float4 *__restrict__ pos_mass, const float4 *__restrict__ sta
     if (step_ctr && tid == FORCE_THREADS - 1 && blockIdx.x == 0 && blockIdx.y == 0) step_ctr[1] = step_ctr[0];
 
     // equal masses <=> no body stamped this launch's generation (stage_sources_kernel); uniform over the grid
-    const bool eqm = __ldg(mass_flag) != generation;
+    const bool eqm = __ldcg(mass_flag) != generation;
     force_tiles<IP, TJ, NST, POT>(eqm, smem_raw, full_bar, empty_bar, acc2, src, tiles_per_split, nx, ny, nz, eps2_2);
-    const float m_common = eqm ? __ldg(pos_mass).w : 1.0f;      // applied once to the finished sums
+    const float m_common = eqm ? __ldcg(pos_mass).w : 1.0f;      // applied once to the finished sums
 
     float4 *o = out + (size_t)blockIdx.y * out_stride;
     const float rinv_eps = rsqrt_approx(eps2);
@@ -340,7 +340,7 @@ __device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partia
             float4 q[REDUCE_CHUNK];
 #pragma unroll
             for (int k = 0; k < REDUCE_CHUNK; ++k)
-                q[k] = k0 + k < splits ? partial[(size_t)(k0 + k) * stride + t] : make_float4(0.f, 0.f, 0.f, 0.f);
+                q[k] = k0 + k < splits ? __ldcg(partial + (size_t)(k0 + k) * stride + t) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
             for (int k = 0; k < REDUCE_CHUNK; ++k) {
                 sx += (double)q[k].x;
@@ -356,7 +356,7 @@ __device__ __forceinline__ float4 sum_partials(const float4 *__restrict__ partia
         float4 q[REDUCE_CHUNK];
 #pragma unroll
         for (int k = 0; k < REDUCE_CHUNK; ++k)
-            q[k] = k0 + k < splits ? partial[(size_t)(k0 + k) * stride + t] : make_float4(0.f, 0.f, 0.f, 0.f);
+            q[k] = k0 + k < splits ? __ldcg(partial + (size_t)(k0 + k) * stride + t) : make_float4(0.f, 0.f, 0.f, 0.f);
         if (k0 == 0) s = q[0];
 #pragma unroll
         for (int k = 0; k < REDUCE_CHUNK; ++k) {

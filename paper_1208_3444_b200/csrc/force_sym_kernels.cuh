@@ -192,7 +192,7 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
     const int a = PART ? a_begin + (int)blockIdx.x : (int)blockIdx.x, s = blockIdx.y;
     if (BODY != 0) {                 // uniform over the grid; before any barrier or copy is set up
         griddep_wait();
-        if ((__ldg(mass_flag) != generation) != (BODY == 2)) return;
+        if ((__ldcg(mass_flag) != generation) != (BODY == 2)) return;
     }
     const int P = TPB * (k_count + (with_plain ? ((nb & 1) ? 1 : 2) : 0));
     const int p0 = (int)(((int64_t)s * P) / splits), p1 = (int)(((int64_t)(s + 1) * P) / splits);
@@ -224,7 +224,7 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
 #pragma unroll
     for (int i = 0; i < IP; ++i) {
         const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
-        const float4 b0 = __ldg(staged + t), b1 = __ldg(staged + t + 1);
+        const float4 b0 = __ldcg(staged + t), b1 = __ldcg(staged + t + 1);
         nx[i] = pack2(-b0.x, -b1.x);
         ny[i] = pack2(-b0.y, -b1.y);
         nz[i] = pack2(-b0.z, -b1.z);
@@ -236,8 +236,8 @@ force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_be
     float *racc = racc_all + (size_t)warp * 3 * TJ;
     for (int j = lane; j < 3 * TJ; j += 32) racc[j] = 0.f;
     if (step_ctr && tid == FORCE_THREADS - 1 && blockIdx.x == 0 && s == 0) step_ctr[1] = step_ctr[0];
-    const bool eqm = __ldg(mass_flag) != generation;
-    const float m_common = eqm ? __ldg(staged).w : 1.0f;        // applied once to the finished sums
+    const bool eqm = __ldcg(mass_flag) != generation;
+    const float m_common = eqm ? __ldcg(staged).w : 1.0f;        // applied once to the finished sums
     __syncwarp();
 
     for (int p = p0; p < p1; ++p) {
@@ -459,7 +459,7 @@ force_sym_pot_kernel(const float4 *__restrict__ staged, int nb, int splits, int 
     const int a = PART ? a_begin + (int)blockIdx.x : (int)blockIdx.x, s = blockIdx.y;
     if (BODY != 0) {                 // uniform over the grid; before any barrier or copy is set up
         griddep_wait();
-        if ((__ldg(mass_flag) != generation) != (BODY == 2)) return;
+        if ((__ldcg(mass_flag) != generation) != (BODY == 2)) return;
     }
     const int P = TPB * (k_count + (with_plain ? ((nb & 1) ? 1 : 2) : 0));
     const int p0 = (int)(((int64_t)s * P) / splits), p1 = (int)(((int64_t)(s + 1) * P) / splits);
@@ -491,7 +491,7 @@ force_sym_pot_kernel(const float4 *__restrict__ staged, int nb, int splits, int 
 #pragma unroll
     for (int i = 0; i < IP; ++i) {
         const int64_t t = tbase + (int64_t)i * (2 * FORCE_THREADS);
-        const float4 b0 = __ldg(staged + t), b1 = __ldg(staged + t + 1);
+        const float4 b0 = __ldcg(staged + t), b1 = __ldcg(staged + t + 1);
         nx[i] = pack2(-b0.x, -b1.x);
         ny[i] = pack2(-b0.y, -b1.y);
         nz[i] = pack2(-b0.z, -b1.z);
@@ -503,8 +503,8 @@ force_sym_pot_kernel(const float4 *__restrict__ staged, int nb, int splits, int 
     float *racc = racc_all + (size_t)warp * NC * TJ;
     for (int j = lane; j < NC * TJ; j += 32) racc[j] = 0.f;
     if (step_ctr && tid == FORCE_THREADS - 1 && blockIdx.x == 0 && s == 0) step_ctr[1] = step_ctr[0];
-    const bool eqm = __ldg(mass_flag) != generation;
-    const float m_common = eqm ? __ldg(staged).w : 1.0f;        // applied once to the finished sums
+    const bool eqm = __ldcg(mass_flag) != generation;
+    const float m_common = eqm ? __ldcg(staged).w : 1.0f;        // applied once to the finished sums
     __syncwarp();
 
     for (int p = p0; p < p1; ++p) {
