@@ -43,12 +43,13 @@ FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.
 # summarised in profiles/: valid only for the (n, source splits) it was captured at -- reported as null otherwise.
 FORCE_KERNEL_DRAM_TRAFFIC = {"bytes": 129934336, "n": 1 << 20, "splits": 8, "symmetric": 0,
                              "profile": "profiles/r02_force_kernel_ncu_full.txt"}
-SYM_KERNEL_DRAM_TRAFFIC = {"bytes": 254605824 + 2335484000, "n": 1 << 20, "splits": 15,
-                           "profile": "profiles/r02_force_sym_kernel_ncu_full.txt"}
+SYM_KERNEL_DRAM_TRAFFIC = {"bytes": 287398912 + 3657097984, "n": 1 << 20, "splits": 15, "launches": 8,
+                           "profile": "profiles/r03_force_sym_kernel_cfg4_chunks.csv (sum over the 8 launches of one "
+                                      "evaluation)"}
 # sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active of the same captures (the hardware counter beside the
 # modelled lane-op figure)
 FORCE_KERNEL_FMA_PIPE_NCU = {"value": 0.883, "profile": "profiles/r02_force_kernel_ncu_full.txt"}
-SYM_KERNEL_FMA_PIPE_NCU = {"value": 0.837, "profile": "profiles/r02_force_sym_kernel_ncu_full.txt"}
+SYM_KERNEL_FMA_PIPE_NCU = {"value": 0.8366, "profile": "profiles/r03_force_sym_kernel_cfg4_chunk_ncu_full.txt"}
 # executed floating-point operations per pair interaction (SASS count): 3 add + 3 mul + 6 fma
 # (x2) + 1 rsqrt = 19 in the general loop, 18 in the equal-mass loop -- beside the 20-flop BASELINE convention
 EXECUTED_FLOP_GENERAL, EXECUTED_FLOP_EQUAL_MASS = 19.0, 18.0
@@ -83,6 +84,10 @@ def parse():
     ap.add_argument("--only-step-loop", type=int, default=0, choices=[0, 1, 2, 3],
                     help="profiling aid: run only the colatus_run step loop of this configuration (optionally with --n) "
                          "and print its steps/s as one JSON line -- the launches ncu captures for the small-N kernels")
+    ap.add_argument("--symmetric-rows", type=int, default=0,
+                    help="measurement aid: cap on the partial rows one launch of the symmetric kernel may use "
+                         "(colatus_set_option symmetric_rows; 0 = what the workspace holds) -- the sweep behind the "
+                         "default row budget, profiles/r03_workspace_rows_sweep.md")
     ap.add_argument("--sharded-driver", action="store_true",
                     help="run the multi-GPU step driver (sharded.py) even at N = 1: a self-test of that code path on one GPU")
     return ap.parse_args()
@@ -289,6 +294,8 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
     cosmo = inputs.Cosmology(H0=float(np.sqrt(8.0 * np.pi / 3.0)), Om_M=1.0)     # EdS, as config 1
     sess = Session(cfg.G, n, device=local_rank)
     begin, count = partition(n, world, rank)
+    if args.symmetric_rows:
+        B.colatus_set_option("symmetric_rows", args.symmetric_rows)
     sess.upload(pm, vel, cfg.eps2)
     tr_idx = (np.arange(N_TRACERS, dtype=np.int64) * (n // N_TRACERS)).astype(np.int32)
     stepper = None
@@ -358,10 +365,12 @@ def measure(args, config_index, n_override, steps, warmup, world, rank, local_ra
     algorithmic_bytes = 32 * n
     if sym:
         cap = SYM_KERNEL_DRAM_TRAFFIC
-        traffic = cap["bytes"] if (cap and n == cap["n"] and world == 1 and plan["splits"] == cap["splits"]) else None
+        traffic = cap["bytes"] if (cap and n == cap["n"] and world == 1 and plan["splits"] == cap["splits"] and
+                                   plan["launches"] == cap.get("launches", 1)) else None
         executed, lane_ops = sym_work(geo["targets_per_thread"], equal_mass)
-        # workspace traffic the method does not ask for: the staged copy and every partial row, written once
-        workspace_bytes_written = 16 * plan["padded_bodies"] * (1 + plan["splits"] + plan["distances"])
+        # workspace traffic the method does not ask for: the staged copy, the target-side rows of the splits (once per
+        # launch) and one reaction row per block distance
+        workspace_bytes_written = 16 * plan["padded_bodies"] * (1 + plan["splits"] * plan["launches"] + plan["distances"])
         pipe_ncu = SYM_KERNEL_FMA_PIPE_NCU if traffic else None
         kernel = "force_sym_kernel<%d,%d,4,%d,%s> (every pair once, applied to both bodies)%s%s" % (
             geo["targets_per_thread"] // 2, 256 if geo["targets_per_thread"] == 4 else 512,

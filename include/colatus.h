@@ -92,9 +92,12 @@ typedef struct colatus_cosmo { double H0, Om_R, Om_M, Om_K, Om_L; } colatus_cosm
  * source array, the partial-sum rows, reduction scratch, and staging for the host-buffer
  * entry point.  From 20480 bodies on the partial rows are those of the symmetric force kernel
  * (colatus_force_plan): one row of 16 bytes per body for every source split and every block
- * distance, capped at 8 GiB -- 0.13 GB at n = 131072, 2.6 GB at 2^20, 8.9 GB at 2^22 (about
- * 1.1 KB per body below 20480).  Non-decreasing in n_max: a workspace sized for n_max serves
- * every n <= n_max.  Pure host arithmetic; 0 if n_max < 1. */
+ * distance while that fits 512 MiB, else 32 rows, the evaluation then taking several launches
+ * (measured cost of the smaller budget: +0.7 % at 2^20, +0.4 % at 2^22).  About 1.1 to 1.4 KB per
+ * body up to 65536 bodies (5.5 MiB at n = 4096, 37 MiB at 32768), 91 MiB at 131072, 0.55 GiB at
+ * 524288, 0.59 GiB at 2^20, 2.36 GiB at 2^22, 9.4 GiB at 2^24 (0.6 KB per body from 2^20 on).
+ * The size depends on n_max alone (not on the device or on options).  Non-decreasing in n_max: a
+ * workspace sized for n_max serves every n <= n_max.  Pure host arithmetic; 0 if n_max < 1. */
 size_t colatus_workspace_bytes(int64_t n_max);
 
 /* Selects the device, checks it is cc 10.x, records G and the workspace.  A second
@@ -365,8 +368,9 @@ int colatus_force_geometry(int64_t n, int64_t target_count, int64_t out[8]);
  * blocks a+1 .. a+distances (mod blocks) both ways, and itself (and the antipodal block when `blocks` is even)
  * one way.  The sums a block receives from each distance are kept as partial rows in the workspace and
  * added in fixed row order (in FP64 when there are more than 16 rows), so results are reproducible bit for
- * bit; when the rows of all distances exceed 8 GiB the evaluation runs as `launches` kernel launches of
- * `distances_per_launch` distances each.  Potential evaluations (with_potential != 0) carry the potential as a
+ * bit; when the rows of all distances exceed the workspace's row budget (512 MiB, or 32 rows if that is more:
+ * from 2^20 bodies on) the evaluation runs as `launches` kernel launches of `distances_per_launch` distances each,
+ * whose sums are carried in FP64 and rounded once.  Potential evaluations (with_potential != 0) carry the potential as a
  * fourth component through the same kernel, always with 1024-body blocks.  Target sub-ranges and smaller
  * problems take the one-directional kernel (out[0] = 0; its geometry is colatus_force_geometry's).
  * out[0] = 1 symmetric / 0 one-directional, out[1] = blocks, out[2] = splits of a block's work (CTAs = blocks x

@@ -49,8 +49,13 @@ constexpr int64_t SYM_WIDE_N = SYM_MID_N;
 constexpr int64_t SYM_MIN_N = 20480;   // measured: faster than force_kernel from here on (profiles/r02_symmetric_kernel.md)
 constexpr int SYM_MAX_SPLITS = 32;
 constexpr int64_t SYM_PAIR_N = 98304;                            // from here on: one kernel per tile body (launch_force_sym)
-constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch can always hold
-constexpr size_t SYM_ROWS_BUDGET = (size_t)8 << 30;               // bytes of partial rows before an evaluation is chunked
+constexpr int SYM_MIN_ROWS = 32;                                  // reaction rows a launch of the 1024 / 1536-body variants can always hold
+// Row budget of the wide (4096-body) variant: all rows of an evaluation while they fit 512 MiB, else 32 rows (splits +
+// block distances per launch), the evaluation then being chunked over block distances.  Measured knee
+// (profiles/r03_workspace_rows_sweep.md): N = 2^20 takes 293.3 ms with all 142 rows (2.4 GB) and 295.3 ms (+0.7 %) with
+// 32 rows (0.5 GB, 8 launches); N = 2^22 4673 ms with 128 rows (8 GiB) and 4690 ms (+0.4 %) with 32 (2 GiB, 27 launches).
+constexpr size_t SYM_ROWS_BUDGET = (size_t)512 << 20;
+constexpr int SYM_BUDGET_ROWS = 32;
 
 struct Geometry {
     int IP = 0, TJ = 0;   // target pairs per thread, sources per tile
@@ -67,7 +72,7 @@ struct Geometry {
 };
 
 struct Workspace {     // byte offsets inside the caller's workspace
-    size_t packed = 0, partials = 0, scratch_acc = 0, trace_slot = 0, diag = 0, stage_in = 0, stage_out = 0,
+    size_t packed = 0, partials = 0, scratch_acc = 0, acc64 = 0, trace_slot = 0, diag = 0, stage_in = 0, stage_out = 0,
            step_table = 0, step_ctr = 0, total = 0;
     static constexpr size_t mass_flag = 0;   // first 256 bytes of the workspace: fixed place for every n
 };
@@ -155,20 +160,26 @@ inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int max_splits(int64_t n) { return n <= SMALL_N ? MAX_SPLITS : MAX_SPLITS_LARGE; }
 
 // Bytes of partial-sum rows for n bodies: the source-split partials of force_kernel, and for n >= SYM_MIN_N the
-// rows of force_sym_kernel -- all of them ((splits + H) rows of n_pad bodies) while that stays within
-// SYM_ROWS_BUDGET, else the budget (the evaluation is then chunked over block distances), never fewer than
-// SYM_MAX_SPLITS + SYM_MIN_ROWS rows.  Non-decreasing in n, so a workspace sized for n_max serves every n <= n_max.
+// rows of force_sym_kernel -- all of them ((splits + H) rows of n_pad bodies) while that stays within the budget,
+// else the budget (the evaluation is then chunked over block distances).  Non-decreasing in n, so a workspace
+// sized for n_max serves every n <= n_max.
 inline int sym_ip(int64_t n) { return g.sym_block ? g.sym_block / 512 : (n < SYM_MID_N ? 2 : (n < SYM_WIDE_N ? 3 : 8)); }
 inline int64_t sym_blocks(int64_t n, int ip) { return (n + 512 * ip - 1) / (512 * ip); }
 size_t sym_rows_bytes(int64_t n, int ip) {
     const size_t row = (size_t)sym_blocks(n, ip) * 512 * ip * 16;
-    size_t bytes = (SYM_MAX_SPLITS + 2) * row;                      // tiny n with "symmetric" = 2
+    size_t bytes = ((ip > 3 ? 24 : SYM_MAX_SPLITS) + 2) * row;      // tiny n with "symmetric" = 2: every split count
     if (n >= SYM_MIN_N) {
         const size_t H = (size_t)((sym_blocks(n, ip) - 1) / 2);
-        size_t want = (SYM_MAX_SPLITS + H) * row;
-        if (want > SYM_ROWS_BUDGET) want = SYM_ROWS_BUDGET;
-        const size_t least = (size_t)(SYM_MAX_SPLITS + SYM_MIN_ROWS) * row;
-        if (want < least) want = least;
+        size_t want;
+        if (ip > 3) {               // wide variant (n >= SYM_WIDE_N): up to 24 splits; budget as above
+            want = (24 + H) * row;
+            const size_t budget = SYM_ROWS_BUDGET > SYM_BUDGET_ROWS * row ? SYM_ROWS_BUDGET : SYM_BUDGET_ROWS * row;
+            if (want > budget) want = budget;
+        } else {                    // automatic below SYM_WIDE_N only (rows of at most 1 MiB): 64 rows hold every plan
+            want = (SYM_MAX_SPLITS + H) * row;
+            const size_t least = (size_t)(SYM_MAX_SPLITS + SYM_MIN_ROWS) * row;
+            if (want < least) want = least;
+        }
         if (want > bytes) bytes = want;
     }
     return bytes;
@@ -192,6 +203,7 @@ Workspace workspace_layout(int64_t n_max) {
     w.packed = off;      off += round_up(n_pad * 16, 256);
     w.partials = off;    off += round_up(partials_bytes(n_max), 256);
     w.scratch_acc = off; off += round_up(n * 16, 256);
+    w.acc64 = off;       off += round_up(n * 24, 256);      // FP64 running sums of chunked symmetric evaluations
     w.trace_slot = off;  off += round_up(n * 4, 256);
     w.diag = off;        off += round_up((size_t)(DIAG_BLOCKS_MAX + 2) * DIAG_Q * 8, 256);
     w.stage_in = off;    off += round_up(n * 16, 256);
@@ -541,12 +553,24 @@ int run_forces(const float4 *pos_mass, int64_t n, int64_t t_begin, int64_t t_cou
             else if (potential)
                 reduce_sym_pot_more_kernel<<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
                                                                    (float)g.G, out);
-            else if (c == 0)
+            else if (geo.chunks == 1)
                 reduce_partials_kernel<false, false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
                                                                              (float)g.G, eps2, pos_mass, 0, out);
-            else
-                reduce_partials_kernel<false, true><<<blocks, 256, 0, st>>>(partials, geo.n_pad, geo.splits + k_count, n,
-                                                                            (float)g.G, eps2, pos_mass, 0, out);
+            else {
+                // chunked: the chunks' row sums are carried in FP64 (workspace) and rounded once, with the last chunk,
+                // so the number of chunks -- the row budget -- does not show in the result's error
+                double *acc64 = reinterpret_cast<double *>(g.ws + w.acc64);
+                const int rows = geo.splits + k_count;
+                if (c == 0)
+                    reduce_partials_chunk_kernel<true, false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, rows, n,
+                                                                                      (float)g.G, acc64, out);
+                else if (c + 1 < geo.chunks)
+                    reduce_partials_chunk_kernel<false, false><<<blocks, 256, 0, st>>>(partials, geo.n_pad, rows, n,
+                                                                                       (float)g.G, acc64, out);
+                else
+                    reduce_partials_chunk_kernel<false, true><<<blocks, 256, 0, st>>>(partials, geo.n_pad, rows, n,
+                                                                                      (float)g.G, acc64, out);
+            }
             CUDA_TRY(cudaGetLastError());
             g.launches++;
         }

@@ -397,4 +397,42 @@ __global__ void __launch_bounds__(256) reduce_partials_kernel(const float4 *__re
     out[t] = r;
 }
 
+// ---- chunked symmetric evaluations: one reduction per chunk of block distances -----------------------
+// The rows of chunk c (the target-side rows of the splits, then the chunk's reaction rows) are added in row order in
+// FP64 and carried across chunks in acc64[t][3] (workspace); the LAST chunk rounds the total once to FP32 and applies
+// G.  FIRST starts the running sum.  Fixed order throughout: same bits every run.
+template <bool FIRST, bool LAST>
+__global__ void __launch_bounds__(256) reduce_partials_chunk_kernel(const float4 *__restrict__ partial, int64_t stride,
+                                                                   int rows, int64_t t_count, float G,
+                                                                   double *__restrict__ acc64,
+                                                                   float4 *__restrict__ out) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= t_count) return;
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    if (!FIRST) {
+        sx = acc64[3 * t];
+        sy = acc64[3 * t + 1];
+        sz = acc64[3 * t + 2];
+    }
+    for (int k0 = 0; k0 < rows; k0 += REDUCE_CHUNK) {
+        float4 q[REDUCE_CHUNK];
+#pragma unroll
+        for (int k = 0; k < REDUCE_CHUNK; ++k)
+            q[k] = k0 + k < rows ? __ldcg(partial + (size_t)(k0 + k) * stride + t) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int k = 0; k < REDUCE_CHUNK; ++k) {
+            sx += (double)q[k].x;
+            sy += (double)q[k].y;
+            sz += (double)q[k].z;
+        }
+    }
+    if (LAST) {
+        out[t] = make_float4((float)sx * G, (float)sy * G, (float)sz * G, 0.f);
+    } else {
+        acc64[3 * t] = sx;
+        acc64[3 * t + 1] = sy;
+        acc64[3 * t + 2] = sz;
+    }
+}
+
 }  // namespace colatus

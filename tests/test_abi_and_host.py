@@ -68,14 +68,18 @@ def test_workspace_bytes_is_host_arithmetic():
     # below 20480 bodies: staged copy + 64 split partials + scratch: ~1.1 KB per body
     w4k = B.colatus_workspace_bytes(4096)
     assert w4k % 256 == 0 and 64 * 16 * 4096 < w4k < 8 * (1 << 20)
-    # symmetric kernel (colatus_force_plan): (32 + 127) partial rows of 256 x 4096 bodies at 2^20 ...
+    # symmetric kernel (colatus_force_plan): all partial rows while they fit 512 MiB ((24 + 31) rows of 64 x 4096
+    # bodies at 262144) ...
+    w18 = B.colatus_workspace_bytes(1 << 18)
+    rows18 = (24 + 31) * 64 * 4096 * 16
+    assert w18 % 256 == 0 and rows18 < w18 < rows18 + 30 * (1 << 20)
+    # ... beyond that 32 rows per launch, the evaluation chunked over block distances (measured knee,
+    # profiles/r03_workspace_rows_sweep.md): VERDICT r2 bounds 0.6 GiB at 2^20, 2.5 GiB at 2^22
     w20, w22 = B.colatus_workspace_bytes(1 << 20), B.colatus_workspace_bytes(1 << 22)
-    rows20 = (32 + 127) * 256 * 4096 * 16
-    assert w20 % 256 == 0 and rows20 < w20 < rows20 + 100 * (1 << 20)
-    # ... capped at 8 GiB of rows (the evaluation is then chunked over block distances)
-    assert (8 << 30) < w22 < (8 << 30) + 400 * (1 << 20)
+    assert w20 % 256 == 0 and (512 << 20) < w20 <= int(0.6 * (1 << 30))
+    assert (2 << 30) < w22 <= int(2.5 * (1 << 30))
     # non-decreasing in n: a workspace sized for n_max serves every n <= n_max
-    sizes = [B.colatus_workspace_bytes(n) for n in (1, 100, 4096, 20479, 20480, 24576, 32768, 65535, 65536, 131071, 131072, 200000, 1 << 20, 1500000, 1 << 22)]
+    sizes = [B.colatus_workspace_bytes(n) for n in (1, 100, 4096, 20479, 20480, 24576, 32768, 65535, 65536, 131071, 131072, 200000, 262144, 400000, 524288, 1 << 20, 1500000, 1 << 22)]
     assert all(a <= b for a, b in zip(sizes, sizes[1:]))
 
 

@@ -231,17 +231,20 @@ def test_plan_of_the_baseline_configurations(session):
     if True:
         small = B.colatus_force_plan(4096)
         assert small["symmetric"] == 0
-        for n in (32768, 100000, 131072, 1 << 20):
+        for n in (32768, 100000, 131072, 262144):                                # all rows fit the 512 MiB budget
             p = B.colatus_force_plan(n)
             block = 1024 if n < 65536 else 4096
             assert p["symmetric"] == 1 and p["launches"] == 1 and p["blocks"] == (n + block - 1) // block
             assert p["partial_rows"] == p["splits"] + p["distances"]
-        big = B.colatus_force_plan(1 << 22)
-        assert big["symmetric"] == 1 and big["launches"] > 1
-        assert big["partial_rows"] * big["padded_bodies"] * 16 <= 8 << 30
+        for n, row_bytes in ((1 << 20, 512 << 20), (1 << 22, 2 << 30)):          # beyond it: 32 rows per launch
+            big = B.colatus_force_plan(n)
+            assert big["symmetric"] == 1 and big["launches"] > 1 and big["partial_rows"] == 32
+            assert big["partial_rows"] == big["splits"] + big["distances_per_launch"]
+            assert big["partial_rows"] * big["padded_bodies"] * 16 == row_bytes
         assert B.colatus_force_plan(1 << 20, 1 << 19)["symmetric"] == 0          # target sub-range
         pot = B.colatus_force_plan(1 << 20, None, True)                          # potential: 1024-body blocks, chunked
-        assert pot["symmetric"] == 1 and pot["blocks"] == 1024 and pot["launches"] == 4
+        assert pot["symmetric"] == 1 and pot["blocks"] == 1024 and pot["launches"] > 1
+        assert pot["partial_rows"] * pot["padded_bodies"] * 16 <= 512 << 20
 
 
 @pytest.mark.parametrize("seed", range(16))

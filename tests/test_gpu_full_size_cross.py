@@ -12,8 +12,8 @@ from conftest import record_parity  # noqa: E402
 
 @pytest.mark.parametrize("index", [4, 5])
 def test_full_size_both_kernels_agree_on_every_target(index):
-    """BASELINE configs 4 (N = 2^20, the launch configuration bench.py times: 256 blocks of 4096 bodies, one launch)
-    and 5 (N = 2^22: 1024 blocks, several launches of block distances): the oracle can check 4096 sampled targets (test_gpu_forces.py);
+    """BASELINE configs 4 (N = 2^20, the launch configuration bench.py times: 256 blocks of 4096 bodies, 8 launches of
+    17 block distances) and 5 (N = 2^22: 1024 blocks, 27 launches): the oracle can check 4096 sampled targets (test_gpu_forces.py);
     here EVERY target is compared between the symmetric and the one-directional kernel -- two independent
     decompositions of eq. (1) -- so that no block, tile, split or chunk boundary of the full-size geometry can hide
     between the samples."""
@@ -23,7 +23,9 @@ def test_full_size_both_kernels_agree_on_every_target(index):
     with Session(1.0, cfg.n) as s:
         d = s.to_device(pm)
         plan = B.colatus_force_plan(cfg.n)
-        assert plan["symmetric"] == 1 and plan["blocks"] == cfg.n // 4096 and (plan["launches"] == 1) == (index == 4)
+        # 32 partial rows per launch (the row budget, profiles/r03_workspace_rows_sweep.md): 15 / 13 splits + 17 / 19 distances
+        assert plan["symmetric"] == 1 and plan["blocks"] == cfg.n // 4096 and plan["partial_rows"] == 32
+        assert plan["launches"] == {4: 8, 5: 27}[index], plan
         sym = s.forces(d, cfg.eps2)
         B.colatus_set_option("symmetric", 0)
         plain = s.forces(d, cfg.eps2)
