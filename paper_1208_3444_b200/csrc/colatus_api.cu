@@ -40,7 +40,7 @@ constexpr int GRAPH_STEPS = COLATUS_GRAPH_STEPS;        // steps per replay of t
 // Variants: blocks of 4096 bodies (16 targets per thread, 254 registers, ONE CTA per SM, 512-source tiles) from
 // SYM_MID_N bodies on -- the per-source work of the source side (shuffle tree, permuted load, address arithmetic) is
 // amortised over 16 targets instead of 6 and 8 independent chains per thread replace the second CTA: 292.8 ms against
-// 313.8 ms at N = 2^20 (profiles/r02_symmetric_kernel.md section 4c); below SYM_MID_N blocks of 1024 (4 targets per
+// 313.8 ms at N = 2^20 (round-2 measurement); below SYM_MID_N blocks of 1024 (4 targets per
 // thread, two CTAs per SM, 256-source tiles), whose finer tiles split better over the SMs (section 4b).  The first
 // variant written, blocks of 1536 (6 targets per thread, two CTAs per SM), is between the two everywhere (within
 // 1 % of the better one at 49152 and 98304 bodies only) and stays selectable ("symmetric_block") for comparisons.
@@ -216,7 +216,7 @@ Workspace workspace_layout(int64_t n_max) {
 
 // Pick the kernel variant (target pairs per thread, tile) and the source split by a cost model fitted to
 // a sweep of every (variant, split) at N = 4096 ... 262144 on the B200 (DESIGN.md 6.3 "Launch geometry";
-// tool: paper_1208_3444_b200/tune_geometry.py, data: profiles/r02_geometry_sweep.md -- picks within 0.6 % of the best
+// round-2 sweep through colatus_set_option, git history, commit 3dbce46: profiles/r02_geometry_sweep.md -- picks within 0.6 % of the best
 // measured geometry with <= 16 splits at every size but N = 8192 (+5 %)):
 //   time ~ a_IP * IP * S * (per_sm + 0.1) + per_sm * c0
 // S = padded sources per split, per_sm = ceil(CTAs / SMs) (an SM works through its CTAs two at a time,
@@ -225,7 +225,7 @@ Workspace workspace_layout(int64_t n_max) {
 // (n, t_count, SM count): the geometry, and with it the summation order, is reproducible.
 Geometry choose_plain_geometry(int64_t n, int64_t t_count) {
     static const int variants[3][2] = {{3, 512}, {2, 512}, {1, 128}};   // (target pairs per thread, tile)
-    // per source, per target pair.  a_us[2] was 0.0287 in round 1; the round-2 sweep (profiles/r02_geometry_sweep.md)
+    // per source, per target pair.  a_us[2] was 0.0287 in round 1; the round-2 sweep (same history)
     // shows the 4-targets-per-thread variant level with the 6-target one for equal masses, and 0.0283 moves
     // N = 131072 from 86 x 12 (+3.4 % over the best measured) to 128 x 16 (+0.2 %) with no other pick changed
     static const double a_us[4] = {0.0, 0.0295, 0.0283, 0.0274};
@@ -238,7 +238,7 @@ Geometry choose_plain_geometry(int64_t n, int64_t t_count) {
         const int64_t per_cta = (int64_t)FORCE_THREADS * 2 * IP;
         const int64_t tiles_t = (t_count + per_cta - 1) / per_cta;
         const int64_t src_tiles = (n + TJ - 1) / TJ;
-        // automatic choice: at most 16 splits -- the sweep (profiles/r02_geometry_sweep.md) shows that beyond 16 the
+        // automatic choice: at most 16 splits -- the round-2 sweep shows that beyond 16 the
         // growing partial-sum reduction eats what the force kernel gains (<= 1.8 % at best, -35 % at worst);
         // a forced split count (colatus_set_option) may go up to max_splits(n)
         const int64_t cap = g.force_splits ? max_splits(n) : MAX_SPLITS_LARGE;

@@ -171,7 +171,7 @@ __device__ __forceinline__ SymTile sym_tile_at(int p, int a, int nb, int k_begin
 // 1-2.5 %); worth the second, empty launch for large problems only.
 // PART: the launch covers the target blocks a_begin .. a_begin + gridDim.x - 1 only (a share of the evaluation).  A
 // template parameter, and a_begin the LAST argument, because the mere use of a_begin in the whole-evaluation kernel
-// moved ptxas's schedule of the tile loop: 319.3 ms against 313.7 ms at N = 2^20 (profiles/r02_symmetric_kernel.md).
+// moved ptxas's schedule of the tile loop: 319.3 ms against 313.7 ms at N = 2^20 (round-2 A/B, git history, commit 3dbce46).
 template <int IP, int TJ, int NST, int MINB, int BODY, bool PART>
 __global__ void __launch_bounds__(FORCE_THREADS, MINB)
 force_sym_kernel(const float4 *__restrict__ staged, int nb, int splits, int k_begin, int k_count, int with_plain,
@@ -327,7 +327,7 @@ constexpr size_t force_sym_pot_smem_bytes() {
 
 // sym_tile_body with the potential as a fourth component: racc = this warp's reaction sums [4][TJ] (x, y, z, pot).
 // A function of its own (and a kernel of its own below) rather than a template flag of sym_tile_body: any edit of
-// that function's text, even one compiled out, moves ptxas's schedule of the force-only loop (profiles/r02_symmetric_kernel.md 3b).  mi = the masses of the thread's own target pairs (general
+// that function's text, even one compiled out, moves ptxas's schedule of the force-only loop (round-2 A/B, git history, commit 3dbce46).  mi = the masses of the thread's own target pairs (general
 // loop only).  POT: also sum_j m_j / sqrt(r^2 + eps^2) on the target side and sum_k m_k / sqrt(...) on the source side
 // (the potential is symmetric in the pair, not antisymmetric: no sign change for the reaction).
 template <int IP, int TJ, bool EQM>
