@@ -164,6 +164,8 @@ class ShardedStepper:
                 t = t.to(self.pos.device)
             dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
             d = t.cpu().numpy()
+        # the one line of the method's arithmetic outside the library: colatus_diagnostics forms the centre of mass as
+        # out[13..15] / out[0] per GPU; over ranks the same FP64 division has to follow the all-reduce of both sums
         d[9:12] = d[13:16] / d[0]
         d[12] = step
         return d
